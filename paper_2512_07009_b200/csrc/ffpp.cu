@@ -1,0 +1,469 @@
+// libffpp — host side: ragged-batch scheduler (a0), workspace, C ABI (include/ffpp.h).
+// Build: nvcc -gencode arch=compute_100a,code=sm_100a -lineinfo -O3 -shared -Xcompiler -fPIC
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "ffpp_kernels.cuh"
+
+using namespace ffpp;
+
+namespace {
+
+thread_local std::string g_create_error;
+
+struct DeviceMeta {           // one pinned block + one device block, uploaded with a single copy
+  size_t frames_off, cand_off_off, unit_prefix_off, tile_prefix_off, bytes;
+};
+
+DeviceMeta meta_layout(int max_frames) {
+  DeviceMeta m;
+  size_t o = 0;
+  m.frames_off = o; o += sizeof(FrameDesc) * (size_t)max_frames;
+  o = (o + 15) & ~(size_t)15;
+  m.cand_off_off = o; o += sizeof(int64_t) * ((size_t)max_frames + 1);
+  m.unit_prefix_off = o; o += sizeof(int32_t) * ((size_t)max_frames + 1);
+  m.tile_prefix_off = o; o += sizeof(int32_t) * ((size_t)max_frames + 1);
+  m.bytes = (o + 15) & ~(size_t)15;
+  return m;
+}
+
+}  // namespace
+
+struct ffpp_handle {
+  ffpp_params p;
+  Consts cst;
+  bool half = false;
+  int key_bytes = 8;
+  int sm_count = 148;
+  int max_frame_cand = 0;
+  int64_t max_total_cells = 0;
+  int64_t mask_words_cap = 0;
+  std::string err;
+
+  // device workspace
+  uint8_t* d_meta = nullptr;
+  void* d_surv_keys = nullptr;
+  int* d_counters = nullptr;          // [0,max_frames) survivor counts | [max_frames, 2*max_frames) sorted counts
+  float4* d_sorted_box = nullptr;
+  float* d_sorted_logit = nullptr;
+  int* d_sorted_idx = nullptr;
+  unsigned long long* d_mask = nullptr;
+  int64_t workspace_bytes = 0;
+  // pinned staging for the descriptor table
+  uint8_t* h_meta = nullptr;
+  DeviceMeta ml;
+  cudaEvent_t meta_done = nullptr;    // last descriptor upload has been consumed by the copy engine
+  // geometry of the last batch (skip rebuild + upload when unchanged)
+  int last_B = -1;
+  std::vector<int32_t> last_N, last_dims;
+  int total_units = 0, total_tiles = 0;
+  int64_t total_cand = 0, total_cells = 0;
+  // host-buffer path staging (allocated on first ffpp_run_host)
+  void* d_in = nullptr;
+  ffpp_box* d_out_boxes = nullptr;
+  int* d_out_counts = nullptr;
+  float* d_out_density = nullptr;
+  // stage timing
+  bool timing = false;
+  cudaEvent_t ev[FFPP_NUM_STAGES + 1] = {};
+  bool ev_valid = false;
+
+  int* surv_cnt() const { return d_counters; }
+  int* n_sorted() const { return d_counters + p.max_frames; }
+};
+
+namespace {
+
+int fail(ffpp_handle* h, int code, const std::string& msg) {
+  if (h) h->err = msg; else g_create_error = msg;
+  return code;
+}
+
+int cuda_fail(ffpp_handle* h, cudaError_t e, const char* what) {
+  return fail(h, FFPP_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+#define FFPP_CUDA(h, call)                                   \
+  do {                                                       \
+    cudaError_t e__ = (call);                                \
+    if (e__ != cudaSuccess) return cuda_fail(h, e__, #call); \
+  } while (0)
+
+bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
+int ilog2(int v) { int l = 0; while ((1 << l) < v) ++l; return l; }
+
+int64_t frame_candidates(const ffpp_params& p, int W, int H) {
+  int64_t n = 0;
+  for (int l = 0; l < p.num_levels; ++l) n += (int64_t)W * H / ((int64_t)p.strides[l] * p.strides[l]);
+  return n;
+}
+
+// a0: validate the batch, (re)build the descriptor table + work-list prefixes, upload if the geometry changed.
+int schedule(ffpp_handle* h, int B, const int32_t* N, const int32_t* dims, cudaStream_t stream) {
+  const ffpp_params& p = h->p;
+  if (B == h->last_B && std::memcmp(N, h->last_N.data(), sizeof(int32_t) * B) == 0 &&
+      std::memcmp(dims, h->last_dims.data(), sizeof(int32_t) * 2 * B) == 0)
+    return FFPP_OK;
+  // the previous upload may still be reading the pinned block
+  FFPP_CUDA(h, cudaEventSynchronize(h->meta_done));
+  h->last_B = -1;
+  FrameDesc* fr = reinterpret_cast<FrameDesc*>(h->h_meta + h->ml.frames_off);
+  int64_t* coff = reinterpret_cast<int64_t*>(h->h_meta + h->ml.cand_off_off);
+  int32_t* uoff = reinterpret_cast<int32_t*>(h->h_meta + h->ml.unit_prefix_off);
+  int32_t* toff = reinterpret_cast<int32_t*>(h->h_meta + h->ml.tile_prefix_off);
+  const int smax = p.strides[p.num_levels - 1];
+  const int R = h->cst.radius;
+  int64_t cand = 0, cells = 0, mwords = 0, units = 0, tiles = 0;
+  for (int f = 0; f < B; ++f) {
+    const int W = dims[2 * f], H = dims[2 * f + 1];
+    if (W <= 0 || H <= 0) return fail(h, FFPP_EINVAL, "frame_dims: W and H must be positive");
+    if (W > p.max_frame_w || H > p.max_frame_h) return fail(h, FFPP_ECAPACITY, "frame exceeds max_frame_w/max_frame_h");
+    if (W % smax) return fail(h, FFPP_EINVAL, "W must be a multiple of the largest stride");
+    if (W % p.cell_px || H % p.cell_px) return fail(h, FFPP_EINVAL, "W and H must be multiples of cell_px");
+    FrameDesc d;
+    std::memset(&d, 0, sizeof(d));
+    int64_t n = 0;
+    for (int l = 0; l < p.num_levels; ++l) {
+      const int64_t s2 = (int64_t)p.strides[l] * p.strides[l];
+      if (((int64_t)W * H) % s2) return fail(h, FFPP_EINVAL, "W*H must be a multiple of stride^2 for every level");
+      d.lvl_start[l] = (int32_t)n;
+      d.lvl_gw[l] = W / p.strides[l];
+      n += (int64_t)W * H / s2;
+    }
+    if (n != N[f]) return fail(h, FFPP_EINVAL, "N_per_frame[f] != sum_l W*H/s_l^2");
+    if (h->key_bytes == 4 && n > 65536) return fail(h, FFPP_ECAPACITY, "frame has more than 65536 candidates (32-bit key handle)");
+    if (n > (1 << 20)) return fail(h, FFPP_ECAPACITY, "frame has more than 2^20 candidates");
+    d.cand_off = cand; d.N = (int32_t)n; d.W = W; d.H = H;
+    d.nmax = (int32_t)(n < p.top_k ? n : p.top_k);
+    d.nbmax = (d.nmax + kNmsTile - 1) / kNmsTile;
+    d.mask_off = mwords;
+    d.dens_off = cells;
+    d.gw = W / p.cell_px; d.gh = H / p.cell_px;
+    if (d.gw < R || d.gh < R) return fail(h, FFPP_EINVAL, "density grid smaller than the Gaussian radius");
+    d.tiles_x = (d.gw + K5_TW - 1) / K5_TW; d.tiles_y = (d.gh + K5_TH - 1) / K5_TH;
+    fr[f] = d;
+    coff[f] = cand; uoff[f] = (int32_t)units; toff[f] = (int32_t)tiles;
+    cand += n; cells += (int64_t)d.gw * d.gh; mwords += mask_words(d.nbmax);
+    units += k3_units(d.nbmax); tiles += (int64_t)d.tiles_x * d.tiles_y;
+    if (units > 0x7fffffff || tiles > 0x7fffffff) return fail(h, FFPP_ECAPACITY, "work list too large");
+  }
+  coff[B] = cand; uoff[B] = (int32_t)units; toff[B] = (int32_t)tiles;
+  if (cand > p.max_total_candidates) return fail(h, FFPP_ECAPACITY, "sum N_f exceeds max_total_candidates");
+  if (cells > h->max_total_cells) return fail(h, FFPP_ECAPACITY, "density cells exceed max_total_cells");
+  if (mwords > h->mask_words_cap) return fail(h, FFPP_ECAPACITY, "suppression mask exceeds nms_workspace_bytes");
+  FFPP_CUDA(h, cudaMemcpyAsync(h->d_meta, h->h_meta, h->ml.bytes, cudaMemcpyHostToDevice, stream));
+  FFPP_CUDA(h, cudaEventRecord(h->meta_done, stream));
+  h->last_B = B;
+  h->last_N.assign(N, N + B);
+  h->last_dims.assign(dims, dims + 2 * B);
+  h->total_units = (int)units; h->total_tiles = (int)tiles; h->total_cand = cand; h->total_cells = cells;
+  return FFPP_OK;
+}
+
+template <bool kHalf, typename KeyT>
+int launch_all(ffpp_handle* h, const void* raw, int B, cudaStream_t st, ffpp_box* out_boxes, int32_t* out_counts,
+               float* out_density) {
+  const FrameDesc* frames = reinterpret_cast<const FrameDesc*>(h->d_meta + h->ml.frames_off);
+  const int64_t* coff = reinterpret_cast<const int64_t*>(h->d_meta + h->ml.cand_off_off);
+  const int32_t* uoff = reinterpret_cast<const int32_t*>(h->d_meta + h->ml.unit_prefix_off);
+  const int32_t* toff = reinterpret_cast<const int32_t*>(h->d_meta + h->ml.tile_prefix_off);
+  const Consts& c = h->cst;
+  const bool tm = h->timing;
+  if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[1], st));
+
+  // a1
+  {
+    const int64_t row = kHalf ? 10 : 20;
+    const int64_t nchunks = (h->total_cand * row + K1_CHUNK_BYTES - 1) / K1_CHUNK_BYTES;
+    int64_t grid = (int64_t)h->sm_count * 3;
+    if (grid > nchunks) grid = nchunks;
+    k1_threshold_compact<kHalf, KeyT><<<(unsigned)grid, K1_THREADS, K1_STAGES * K1_CHUNK_BYTES, st>>>(
+        static_cast<const uint8_t*>(raw), h->total_cand, B, coff, c.logit_thr, static_cast<KeyT*>(h->d_surv_keys),
+        h->surv_cnt());
+  }
+  if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[2], st));
+  // a2
+  {
+    const int cap = h->p.top_k;
+    const size_t smem = 2 * (size_t)cap * sizeof(KeyT) + K2_WARPS * 256 * sizeof(uint16_t) + 256 * sizeof(uint32_t) + sizeof(K2Misc);
+    k2_sort_topk_decode<kHalf, KeyT><<<B, K2_THREADS, smem, st>>>(static_cast<const uint8_t*>(raw), frames,
+                                                                   static_cast<const KeyT*>(h->d_surv_keys), h->surv_cnt(), c,
+                                                                   cap, h->d_sorted_box, h->d_sorted_logit, h->d_sorted_idx,
+                                                                   h->n_sorted());
+  }
+  if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[3], st));
+  // a3
+  if (h->total_units > 0)
+    k3_nms_mask<<<h->total_units, K3_THREADS, 0, st>>>(frames, uoff, B, h->d_sorted_box, h->n_sorted(), c, h->d_mask);
+  if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[4], st));
+  // a4
+  {
+    const size_t smem = sizeof(unsigned long long) * (size_t)((h->p.top_k + kNmsTile - 1) / kNmsTile);
+    k4_nms_sweep<<<B, K4_THREADS, smem, st>>>(frames, h->d_sorted_box, h->d_sorted_logit, h->d_sorted_idx, h->n_sorted(), c,
+                                              h->d_mask, out_boxes, out_counts);
+  }
+  if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[5], st));
+  // a5-a6
+  {
+    const int R = c.radius;
+    const size_t smem = sizeof(int) * (size_t)(K5_TH + 2 * R) * (K5_TW + 2 * R) + sizeof(float) * (size_t)(K5_TH + 2 * R) * K5_TW;
+    k5_density<<<h->total_tiles, K5_THREADS, smem, st>>>(frames, toff, B, out_boxes, out_counts, c, out_density);
+  }
+  if (tm) {
+    FFPP_CUDA(h, cudaEventRecord(h->ev[6], st));
+    h->ev_valid = true;
+  }
+  FFPP_CUDA(h, cudaGetLastError());
+  return FFPP_OK;
+}
+
+template <bool kHalf, typename KeyT>
+int set_kernel_attrs(ffpp_handle* h) {
+  const size_t s1 = K1_STAGES * K1_CHUNK_BYTES;
+  FFPP_CUDA(h, cudaFuncSetAttribute(k1_threshold_compact<kHalf, KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s1));
+  const size_t s2 = 2 * (size_t)h->p.top_k * sizeof(KeyT) + K2_WARPS * 256 * sizeof(uint16_t) + 256 * sizeof(uint32_t) + sizeof(K2Misc);
+  FFPP_CUDA(h, cudaFuncSetAttribute(k2_sort_topk_decode<kHalf, KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s2));
+  return FFPP_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int ffpp_create(const ffpp_params* p, ffpp_handle** out) {
+  if (!p || !out) return fail(nullptr, FFPP_EINVAL, "ffpp_create: null argument");
+  if (p->dtype != 0 && p->dtype != 1) return fail(nullptr, FFPP_EINVAL, "dtype must be 0 (fp32) or 1 (fp16)");
+  if (p->num_levels < 1 || p->num_levels > kMaxLevels) return fail(nullptr, FFPP_EINVAL, "num_levels must be 1..4");
+  for (int l = 0; l < p->num_levels; ++l) {
+    if (!is_pow2(p->strides[l])) return fail(nullptr, FFPP_EINVAL, "strides must be powers of two");
+    if (l && p->strides[l] <= p->strides[l - 1]) return fail(nullptr, FFPP_EINVAL, "strides must be ascending");
+  }
+  if (!(p->iou_thresh >= 0.0f)) return fail(nullptr, FFPP_EINVAL, "iou_thresh must be >= 0");
+  if (std::isnan(p->conf_thresh)) return fail(nullptr, FFPP_EINVAL, "conf_thresh is NaN");
+  if (p->top_k < 1) return fail(nullptr, FFPP_EINVAL, "top_k must be >= 1");
+  if (p->cell_px < 1) return fail(nullptr, FFPP_EINVAL, "cell_px must be >= 1");
+  if (!(p->sigma_cells > 0.0f) || !(p->truncate_sigmas > 0.0f)) return fail(nullptr, FFPP_EINVAL, "sigma_cells and truncate_sigmas must be > 0");
+  if (p->max_frames < 1 || p->max_total_candidates < 1 || p->max_frame_w < 1 || p->max_frame_h < 1)
+    return fail(nullptr, FFPP_EINVAL, "capacities must be positive");
+  const int R = (int)std::floor((double)p->truncate_sigmas * (double)p->sigma_cells);
+  if (R < 1 || R > kMaxRadius) return fail(nullptr, FFPP_EINVAL, "Gaussian radius floor(truncate*sigma) must be 1..32");
+
+  ffpp_handle* h = new (std::nothrow) ffpp_handle();
+  if (!h) return fail(nullptr, FFPP_ENOMEM, "host allocation failed");
+  h->p = *p;
+  h->half = p->dtype == 1;
+  const int64_t nmaxframe = frame_candidates(*p, p->max_frame_w, p->max_frame_h);
+  h->max_frame_cand = (int)std::min<int64_t>(nmaxframe, 1 << 20);
+  h->key_bytes = (h->half && nmaxframe <= 65536) ? 4 : 8;
+  const int kcap = h->key_bytes == 4 ? 24576 : 12288;
+  if (p->top_k > kcap) { delete h; return fail(nullptr, FFPP_EINVAL, "top_k exceeds the shared-memory sort capacity (24576 / 12288)"); }
+
+  // constants
+  Consts& c = h->cst;
+  std::memset(&c, 0, sizeof(c));
+  if (!(p->conf_thresh > 0.0f)) c.logit_thr = -INFINITY;
+  else if (!(p->conf_thresh < 1.0f)) c.logit_thr = INFINITY;
+  else c.logit_thr = (float)std::log((double)p->conf_thresh / (1.0 - (double)p->conf_thresh));
+  c.iou_thr = p->iou_thresh;
+  c.iou_fast = (p->iou_thresh >= 1e-6f && p->iou_thresh <= 1e6f) ? 1 : 0;
+  c.iou_thr_hi = std::nextafterf((float)((double)p->iou_thresh * (1.0 + std::ldexp(1.0, -20))), INFINITY);
+  c.iou_thr_lo = std::nextafterf((float)((double)p->iou_thresh * (1.0 - std::ldexp(1.0, -20))), -INFINITY);
+  c.top_k = p->top_k;
+  c.num_levels = p->num_levels;
+  for (int l = 0; l < p->num_levels; ++l) c.stride_log2[l] = ilog2(p->strides[l]);
+  c.cell_px = p->cell_px;
+  c.radius = R;
+  {
+    double Z = 0.0, s2 = 2.0 * (double)p->sigma_cells * (double)p->sigma_cells;
+    for (int k = -R; k <= R; ++k) Z += std::exp(-(double)(k * k) / s2);
+    for (int k = -R; k <= R; ++k) c.taps[k + R] = (float)(std::exp(-(double)(k * k) / s2) / Z);
+  }
+
+  auto bail = [&](int code, const std::string& msg) { ffpp_destroy(h); return fail(nullptr, code, msg); };
+  cudaError_t e;
+  int dev = 0;
+  if ((e = cudaGetDevice(&dev)) != cudaSuccess) return bail(FFPP_ECUDA, std::string("cudaGetDevice: ") + cudaGetErrorString(e));
+  cudaDeviceProp prop;
+  if ((e = cudaGetDeviceProperties(&prop, dev)) != cudaSuccess) return bail(FFPP_ECUDA, std::string("cudaGetDeviceProperties: ") + cudaGetErrorString(e));
+  if (prop.major != 10) return bail(FFPP_ECUDA, "libffpp is built for sm_100a only; this device is sm_" + std::to_string(prop.major * 10 + prop.minor));
+  h->sm_count = prop.multiProcessorCount;
+
+  // capacities
+  const int64_t cells_frame = (int64_t)(p->max_frame_w / p->cell_px) * (p->max_frame_h / p->cell_px);
+  h->max_total_cells = p->max_total_cells > 0 ? p->max_total_cells : cells_frame * p->max_frames;
+  const int nbcap = (int)((std::min<int64_t>(p->top_k, nmaxframe) + kNmsTile - 1) / kNmsTile);
+  h->mask_words_cap = p->nms_workspace_bytes > 0 ? p->nms_workspace_bytes / 8 : mask_words(nbcap) * p->max_frames;
+
+  h->ml = meta_layout(p->max_frames);
+  auto dalloc = [&](void** ptr, size_t bytes) {
+    if (bytes == 0) bytes = 16;
+    cudaError_t ee = cudaMalloc(ptr, bytes);
+    if (ee == cudaSuccess) h->workspace_bytes += (int64_t)bytes;
+    return ee;
+  };
+  const size_t K = (size_t)p->top_k, F = (size_t)p->max_frames;
+  if ((e = dalloc((void**)&h->d_meta, h->ml.bytes)) != cudaSuccess ||
+      (e = dalloc(&h->d_surv_keys, (size_t)p->max_total_candidates * h->key_bytes)) != cudaSuccess ||
+      (e = dalloc((void**)&h->d_counters, 2 * F * sizeof(int))) != cudaSuccess ||
+      (e = dalloc((void**)&h->d_sorted_box, F * K * sizeof(float4))) != cudaSuccess ||
+      (e = dalloc((void**)&h->d_sorted_logit, F * K * sizeof(float))) != cudaSuccess ||
+      (e = dalloc((void**)&h->d_sorted_idx, F * K * sizeof(int))) != cudaSuccess ||
+      (e = dalloc((void**)&h->d_mask, (size_t)h->mask_words_cap * 8)) != cudaSuccess) {
+    cudaGetLastError();
+    return bail(e == cudaErrorMemoryAllocation ? FFPP_ENOMEM : FFPP_ECUDA, std::string("workspace cudaMalloc: ") + cudaGetErrorString(e));
+  }
+  if ((e = cudaMallocHost((void**)&h->h_meta, h->ml.bytes)) != cudaSuccess) return bail(FFPP_ENOMEM, std::string("cudaMallocHost: ") + cudaGetErrorString(e));
+  if ((e = cudaEventCreateWithFlags(&h->meta_done, cudaEventDisableTiming)) != cudaSuccess) return bail(FFPP_ECUDA, std::string("cudaEventCreate: ") + cudaGetErrorString(e));
+  for (int i = 0; i <= FFPP_NUM_STAGES; ++i)
+    if ((e = cudaEventCreate(&h->ev[i])) != cudaSuccess) return bail(FFPP_ECUDA, std::string("cudaEventCreate: ") + cudaGetErrorString(e));
+  int rc;
+  if (h->half && h->key_bytes == 4) rc = set_kernel_attrs<true, uint32_t>(h);
+  else if (h->half) rc = set_kernel_attrs<true, uint64_t>(h);
+  else rc = set_kernel_attrs<false, uint64_t>(h);
+  if (rc != FFPP_OK) { std::string m = h->err; return bail(rc, m); }
+  {
+    const size_t s5 = sizeof(int) * (size_t)(K5_TH + 2 * R) * (K5_TW + 2 * R) + sizeof(float) * (size_t)(K5_TH + 2 * R) * K5_TW;
+    if ((e = cudaFuncSetAttribute(k5_density, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s5)) != cudaSuccess)
+      return bail(FFPP_ECUDA, std::string("cudaFuncSetAttribute(k5): ") + cudaGetErrorString(e));
+  }
+  *out = h;
+  return FFPP_OK;
+}
+
+int ffpp_run(ffpp_handle* h, const void* raw, int32_t B, const int32_t* N_per_frame, const int32_t* frame_dims, void* stream,
+             ffpp_box* out_boxes, int32_t* out_counts, float* out_density) {
+  if (!h) return FFPP_EINVAL;
+  if (B < 0) return fail(h, FFPP_EINVAL, "B < 0");
+  if (B == 0) return FFPP_OK;
+  if (!raw || !N_per_frame || !frame_dims || !out_boxes || !out_counts || !out_density) return fail(h, FFPP_EINVAL, "null pointer");
+  if (B > h->p.max_frames) return fail(h, FFPP_ECAPACITY, "B exceeds max_frames");
+  if (reinterpret_cast<uintptr_t>(raw) & 15) return fail(h, FFPP_EINVAL, "raw must be 16-byte aligned");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  if (h->timing) FFPP_CUDA(h, cudaEventRecord(h->ev[0], st));
+  int rc = schedule(h, B, N_per_frame, frame_dims, st);
+  if (rc != FFPP_OK) return rc;
+  FFPP_CUDA(h, cudaMemsetAsync(h->d_counters, 0, sizeof(int) * 2 * (size_t)h->p.max_frames, st));
+  if (h->half && h->key_bytes == 4) return launch_all<true, uint32_t>(h, raw, B, st, out_boxes, out_counts, out_density);
+  if (h->half) return launch_all<true, uint64_t>(h, raw, B, st, out_boxes, out_counts, out_density);
+  return launch_all<false, uint64_t>(h, raw, B, st, out_boxes, out_counts, out_density);
+}
+
+int ffpp_run_host(ffpp_handle* h, const void* raw, int32_t B, const int32_t* N_per_frame, const int32_t* frame_dims, void* stream,
+                  ffpp_box* out_boxes, int32_t* out_counts, float* out_density) {
+  if (!h) return FFPP_EINVAL;
+  if (B < 0) return fail(h, FFPP_EINVAL, "B < 0");
+  if (B == 0) return FFPP_OK;
+  if (!raw || !N_per_frame || !frame_dims || !out_boxes || !out_counts || !out_density) return fail(h, FFPP_EINVAL, "null pointer");
+  if (B > h->p.max_frames) return fail(h, FFPP_ECAPACITY, "B exceeds max_frames");
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const size_t esz = h->half ? 2 : 4;
+  if (!h->d_in) {  // first use of the host path: its device staging (not part of ffpp_run's no-allocation promise)
+    const size_t K = (size_t)h->p.top_k, F = (size_t)h->p.max_frames;
+    FFPP_CUDA(h, cudaMalloc(&h->d_in, (size_t)h->p.max_total_candidates * 5 * esz + 16));
+    FFPP_CUDA(h, cudaMalloc((void**)&h->d_out_boxes, F * K * sizeof(ffpp_box)));
+    FFPP_CUDA(h, cudaMalloc((void**)&h->d_out_counts, F * sizeof(int)));
+    FFPP_CUDA(h, cudaMalloc((void**)&h->d_out_density, (size_t)h->max_total_cells * sizeof(float)));
+  }
+  int64_t cand = 0, cells = 0;
+  for (int f = 0; f < B; ++f) {
+    cand += N_per_frame[f];
+    cells += (int64_t)(frame_dims[2 * f] / h->p.cell_px) * (frame_dims[2 * f + 1] / h->p.cell_px);
+  }
+  if (cand > h->p.max_total_candidates) return fail(h, FFPP_ECAPACITY, "sum N_f exceeds max_total_candidates");
+  if (cells > h->max_total_cells) return fail(h, FFPP_ECAPACITY, "density cells exceed max_total_cells");
+  FFPP_CUDA(h, cudaMemcpyAsync(h->d_in, raw, (size_t)cand * 5 * esz, cudaMemcpyHostToDevice, st));
+  int rc = ffpp_run(h, h->d_in, B, N_per_frame, frame_dims, stream, h->d_out_boxes, h->d_out_counts, h->d_out_density);
+  if (rc != FFPP_OK) return rc;
+  FFPP_CUDA(h, cudaMemcpyAsync(out_counts, h->d_out_counts, sizeof(int) * (size_t)B, cudaMemcpyDeviceToHost, st));
+  FFPP_CUDA(h, cudaMemcpyAsync(out_density, h->d_out_density, sizeof(float) * (size_t)cells, cudaMemcpyDeviceToHost, st));
+  FFPP_CUDA(h, cudaStreamSynchronize(st));
+  // only rows [0, count) of each frame are defined: copy exactly those
+  const size_t K = (size_t)h->p.top_k;
+  for (int f = 0; f < B; ++f)
+    if (out_counts[f] > 0)
+      FFPP_CUDA(h, cudaMemcpyAsync(out_boxes + (size_t)f * K, h->d_out_boxes + (size_t)f * K, sizeof(ffpp_box) * (size_t)out_counts[f],
+                                   cudaMemcpyDeviceToHost, st));
+  FFPP_CUDA(h, cudaStreamSynchronize(st));
+  return FFPP_OK;
+}
+
+int ffpp_destroy(ffpp_handle* h) {
+  if (!h) return FFPP_OK;
+  cudaFree(h->d_meta); cudaFree(h->d_surv_keys); cudaFree(h->d_counters); cudaFree(h->d_sorted_box);
+  cudaFree(h->d_sorted_logit); cudaFree(h->d_sorted_idx); cudaFree(h->d_mask);
+  cudaFree(h->d_in); cudaFree(h->d_out_boxes); cudaFree(h->d_out_counts); cudaFree(h->d_out_density);
+  if (h->h_meta) cudaFreeHost(h->h_meta);
+  if (h->meta_done) cudaEventDestroy(h->meta_done);
+  for (int i = 0; i <= FFPP_NUM_STAGES; ++i)
+    if (h->ev[i]) cudaEventDestroy(h->ev[i]);
+  delete h;
+  return FFPP_OK;
+}
+
+const char* ffpp_last_error(const ffpp_handle* h) { return h ? h->err.c_str() : g_create_error.c_str(); }
+
+int ffpp_get_info(const ffpp_handle* h, ffpp_info* out) {
+  if (!h || !out) return FFPP_EINVAL;
+  std::memset(out, 0, sizeof(*out));
+  out->logit_threshold = h->cst.logit_thr;
+  out->radius = h->cst.radius;
+  for (int k = 0; k <= 2 * h->cst.radius; ++k) out->taps[k] = h->cst.taps[k];
+  out->key_bits = h->key_bytes * 8;
+  out->workspace_bytes = h->workspace_bytes;
+  out->sm_count = h->sm_count;
+  return FFPP_OK;
+}
+
+int ffpp_set_stage_timing(ffpp_handle* h, int32_t enable) {
+  if (!h) return FFPP_EINVAL;
+  h->timing = enable != 0;
+  h->ev_valid = false;
+  return FFPP_OK;
+}
+
+int ffpp_get_stage_ms(ffpp_handle* h, float* ms_out) {
+  if (!h || !ms_out) return FFPP_EINVAL;
+  if (!h->ev_valid) return fail(h, FFPP_EINVAL, "no timed run recorded");
+  for (int i = 0; i < FFPP_NUM_STAGES; ++i) FFPP_CUDA(h, cudaEventElapsedTime(&ms_out[i], h->ev[i], h->ev[i + 1]));
+  return FFPP_OK;
+}
+
+int ffpp_debug_read(ffpp_handle* h, int32_t what, void* dst, int64_t dst_bytes) {
+  if (!h || !dst) return FFPP_EINVAL;
+  if (h->last_B < 0) return fail(h, FFPP_EINVAL, "no run to read back");
+  const int B = h->last_B;
+  const size_t K = (size_t)h->p.top_k;
+  FFPP_CUDA(h, cudaDeviceSynchronize());
+  if (what == 0 || what == 1) {
+    if (dst_bytes < (int64_t)(sizeof(int) * B)) return fail(h, FFPP_EINVAL, "dst too small");
+    FFPP_CUDA(h, cudaMemcpy(dst, what == 0 ? h->surv_cnt() : h->n_sorted(), sizeof(int) * B, cudaMemcpyDeviceToHost));
+    return FFPP_OK;
+  }
+  std::vector<int> ns((size_t)B);
+  FFPP_CUDA(h, cudaMemcpy(ns.data(), h->n_sorted(), sizeof(int) * B, cudaMemcpyDeviceToHost));
+  if (what == 2) {
+    if (dst_bytes < (int64_t)(sizeof(int) * B * K)) return fail(h, FFPP_EINVAL, "dst too small");
+    int* d = static_cast<int*>(dst);
+    FFPP_CUDA(h, cudaMemcpy(d, h->d_sorted_idx, sizeof(int) * B * K, cudaMemcpyDeviceToHost));
+    for (int f = 0; f < B; ++f)
+      for (size_t k = (size_t)ns[(size_t)f]; k < K; ++k) d[(size_t)f * K + k] = -1;
+    return FFPP_OK;
+  }
+  if (what == 3) {
+    if (dst_bytes < (int64_t)(sizeof(float) * 4 * B * K)) return fail(h, FFPP_EINVAL, "dst too small");
+    float* d = static_cast<float*>(dst);
+    FFPP_CUDA(h, cudaMemcpy(d, h->d_sorted_box, sizeof(float) * 4 * B * K, cudaMemcpyDeviceToHost));
+    for (int f = 0; f < B; ++f)
+      for (size_t k = (size_t)ns[(size_t)f]; k < K; ++k)
+        for (int e = 0; e < 4; ++e) d[((size_t)f * K + k) * 4 + e] = 0.0f;
+    return FFPP_OK;
+  }
+  return fail(h, FFPP_EINVAL, "unknown debug selector");
+}
+
+}  // extern "C"

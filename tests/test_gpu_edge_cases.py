@@ -1,0 +1,172 @@
+"""GPU edge cases: empty / tiny / boundary-size inputs, ties, ABI misuse."""
+import numpy as np
+import pytest
+
+from parity import compare
+
+pytestmark = pytest.mark.gpu
+
+P = dict(dtype="fp16", conf_thresh=0.25, iou_thresh=0.45, top_k=3000, strides=[8, 16, 32], cell_px=8, sigma_cells=2.0,
+         truncate_sigmas=3.0)
+
+
+class W:
+    def __init__(self, raw, dims, params):
+        import flockgen
+        self.raw = raw
+        self.frame_dims = np.asarray(dims, dtype=np.int32).reshape(-1, 2)
+        self.N_per_frame = np.array([flockgen.frame_candidates(int(a), int(b)) for a, b in self.frame_dims], dtype=np.int32)
+        self.params = params
+        assert raw.shape[0] == int(self.N_per_frame.sum())
+
+
+@pytest.fixture(scope="module")
+def env(oracle_mod, gen_mod):
+    torch = pytest.importorskip("torch")
+    assert torch.cuda.is_available()
+    import paper_2512_07009_b200 as m
+    m.load_library()
+    return torch, m, oracle_mod, gen_mod
+
+
+def check(env, w, **kw):
+    torch, m, oracle_mod, _ = env
+    pp = m.FFPP.for_workload(w, **kw)
+    out = pp.run(torch.from_numpy(w.raw).cuda(), w.N_per_frame, w.frame_dims)
+    torch.cuda.synchronize()
+    ref = oracle_mod.run(w.params, w.raw, w.N_per_frame, w.frame_dims)
+    compare(out, ref, w, check_stage=pp)
+    return out, ref
+
+
+def frame(N, dtype, rng, n_pass, spread=600.0, lo=2.0, hi=6.0):
+    """Background frame with n_pass random survivors at random candidates (tie-free unless asked)."""
+    raw = np.zeros((N, 5), dtype=dtype)
+    raw[:, :4] = 1.0
+    raw[:, 4] = -8.0
+    if n_pass:
+        js = rng.choice(N, size=n_pass, replace=False)
+        raw[js, :4] = rng.uniform(0.5, 3.0, size=(n_pass, 4))
+        raw[js, 4] = rng.uniform(lo, hi, size=n_pass)
+    return raw
+
+
+@pytest.mark.parametrize("dt", ["fp16", "fp32"])
+@pytest.mark.parametrize("n_pass", [0, 1, 2, 63, 64, 65, 127, 128, 129, 1000])
+def test_survivor_counts_around_tile_boundaries(env, dt, n_pass):
+    rng = np.random.default_rng(100 + n_pass)
+    npdt = np.float16 if dt == "fp16" else np.float32
+    w = W(frame(8400, npdt, rng, n_pass), [[640, 640]], dict(P, dtype=dt))
+    out, ref = check(env, w)
+    assert ref.survivor_counts[0] == n_pass
+
+
+def test_all_pass_none_pass_and_topk_cut(env):
+    rng = np.random.default_rng(3)
+    raw = frame(8400, np.float16, rng, 0)
+    raw[:, 4] = rng.uniform(-1.0, 8.0, size=8400)      # everything above logit(0.25) = -1.0986
+    raw[:, :4] = rng.uniform(0.2, 1.5, size=(8400, 4))
+    for K in (1, 64, 100, 3000, 8400, 12000):
+        w = W(raw, [[640, 640]], dict(P, top_k=K, iou_thresh=0.6))
+        out, ref = check(env, w)
+        assert ref.survivor_counts[0] == 8400 and ref.sorted_counts[0] == min(K, 8400)
+    w = W(frame(8400, np.float16, rng, 0), [[640, 640]], P)
+    out, ref = check(env, w)
+    assert ref.counts[0] == 0 and not out.density_numpy().any()
+
+
+def test_equal_scores_and_signed_zero_ties(env):
+    rng = np.random.default_rng(4)
+    for dt, npdt in (("fp16", np.float16), ("fp32", np.float32)):
+        raw = frame(8400, npdt, rng, 0)
+        js = rng.choice(8400, size=2000, replace=False)
+        vals = np.array([-0.5, 0.0, -0.0, 0.5, 1.0, 2.0, 3.0], dtype=npdt)
+        raw[js, 4] = vals[rng.integers(0, len(vals), size=2000)]
+        raw[js, :4] = rng.uniform(0.2, 1.0, size=(2000, 4))
+        w = W(raw, [[640, 640]], dict(P, dtype=dt, top_k=777, iou_thresh=1.0))
+        out, ref = check(env, w)
+        assert ref.counts[0] == 777                     # thr >= 1: kept list == sorted top-K list
+
+
+def test_boxes_outside_the_frame_and_border_cells(env):
+    rng = np.random.default_rng(5)
+    raw = frame(8400, np.float32, rng, 0)
+    # survivors along the frame border with large one-sided distances -> centroids outside / on the border cell
+    border = [0, 79, 80 * 79, 6399, 6400, 6439, 8000, 8399, 40, 80 * 40]
+    for k, j in enumerate(border):
+        raw[j] = [30.0 - 3 * k, 0.5, 0.5 + 3 * k, 0.5, 5.0 - 0.1 * k]
+    raw[3000] = [0.5, 40.0, 0.5, 0.25, 6.0]
+    raw[3100] = [0.5, 0.25, 0.5, 60.0, 6.5]
+    w = W(raw, [[640, 640]], dict(P, dtype="fp32", iou_thresh=0.9))
+    out, ref = check(env, w)
+    b = ref.boxes[0, :ref.counts[0]]
+    cx = (b["x1"] + b["x2"]) / 2
+    assert (cx < 0).any() or (cx >= 640).any()          # the case really has out-of-frame centroids
+
+
+def test_720p_partial_row_and_ragged_mix(env):
+    torch, m, oracle_mod, gen = env
+    rng = np.random.default_rng(6)
+    dims = [[1280, 720], [640, 640], [1280, 720], [1920, 1088], [1280, 720], [64, 64]]
+    parts = []
+    for W_, H_ in dims:
+        N = gen.frame_candidates(W_, H_)
+        fr = frame(N, np.float16, rng, min(N // 3, 2500), lo=0.0, hi=8.0)
+        fr[N - 20:, 4] = 9.0                           # the half row of 1280x720 (A21) survives
+        parts.append(fr)
+    w = W(np.concatenate(parts), dims, dict(P, top_k=2000, iou_thresh=0.5, sigma_cells=2.5))
+    check(env, w)
+
+
+def test_many_tiny_frames_take_the_generic_compaction_path(env):
+    torch, m, oracle_mod, gen = env
+    rng = np.random.default_rng(7)
+    dims = [[64, 64]] * 150                              # N = 84 per frame: > 16 frames per 2048-candidate chunk
+    parts = [frame(84, np.float16, rng, int(rng.integers(0, 60)), lo=0.0, hi=8.0) for _ in dims]
+    w = W(np.concatenate(parts), dims, dict(P, top_k=50, sigma_cells=1.0))
+    check(env, w)
+
+
+def test_max_topk_for_both_key_widths(env):
+    rng = np.random.default_rng(8)
+    N = 42840
+    raw = frame(N, np.float16, rng, 0)
+    raw[:, 4] = rng.uniform(-1.0, 8.0, size=N)
+    raw[:, :4] = rng.uniform(0.1, 0.6, size=(N, 4))
+    w = W(raw, [[1920, 1088]], dict(P, top_k=24576, iou_thresh=0.7, sigma_cells=3.0))
+    check(env, w)
+    w32 = W(raw.astype(np.float32), [[1920, 1088]], dict(P, dtype="fp32", top_k=12288, iou_thresh=0.7, sigma_cells=3.0))
+    check(env, w32)
+
+
+def test_abi_misuse_is_rejected(env):
+    torch, m, oracle_mod, gen = env
+    good = dict(max_frames=2, max_total_candidates=2 * 8400, max_frame_w=640, max_frame_h=640)
+    for bad in (dict(P, dtype="fp16", top_k=0), dict(P, strides=[8, 24, 32]), dict(P, iou_thresh=-0.1),
+                dict(P, sigma_cells=0.0), dict(P, top_k=30000), dict(P, strides=[16, 8, 32])):
+        with pytest.raises(m.FFPPError) as ei:
+            m.FFPP(bad, **good)
+        assert ei.value.code == m.FFPP_EINVAL
+    pp = m.FFPP(P, **good)
+    raw = torch.zeros((8400, 5), dtype=torch.float16, device="cuda")
+    out = pp.alloc_outputs(1, [[640, 640]])
+    N = np.array([8400], dtype=np.int32); dims = np.array([[640, 640]], dtype=np.int32)
+    args = lambda **k: dict(dict(raw_ptr=raw.data_ptr(), B=1, N_ptr=N.ctypes.data, dims_ptr=dims.ctypes.data, stream_ptr=None,
+                                 boxes_ptr=out.boxes.data_ptr(), counts_ptr=out.counts.data_ptr(),
+                                 density_ptr=out.density.data_ptr()), **k)
+    assert pp.run_raw_pointers(**args()) == m.FFPP_OK
+    assert pp.run_raw_pointers(**args(B=0)) == m.FFPP_OK
+    assert pp.run_raw_pointers(**args(B=-1)) == m.FFPP_EINVAL
+    assert pp.run_raw_pointers(**args(raw_ptr=None)) == m.FFPP_EINVAL
+    assert pp.run_raw_pointers(**args(boxes_ptr=None)) == m.FFPP_EINVAL
+    assert pp.run_raw_pointers(**args(raw_ptr=raw.data_ptr() + 2)) == m.FFPP_EINVAL and "aligned" in pp.last_error()
+    assert pp.run_raw_pointers(**args(B=3)) == m.FFPP_ECAPACITY
+    badN = np.array([8399], dtype=np.int32)
+    assert pp.run_raw_pointers(**args(N_ptr=badN.ctypes.data)) == m.FFPP_EINVAL
+    for d in ([[648, 640]], [[640, 644]], [[1280, 1280]]):
+        dd = np.array(d, dtype=np.int32)
+        nn = np.array([gen.frame_candidates(*d[0])], dtype=np.int32)
+        rc = pp.run_raw_pointers(**args(dims_ptr=dd.ctypes.data, N_ptr=nn.ctypes.data))
+        assert rc in (m.FFPP_EINVAL, m.FFPP_ECAPACITY) and rc != m.FFPP_OK
+    torch.cuda.synchronize()
+    pp.close()

@@ -1,0 +1,97 @@
+"""GPU parity: the CUDA path (through the C ABI) against the oracle on the same seeded inputs."""
+import numpy as np
+import pytest
+
+from parity import compare
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    torch = pytest.importorskip("torch")
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def ffpp_mod():
+    import paper_2512_07009_b200 as m
+    m.load_library()          # raises if the extension cannot be built/loaded: no silent fallback
+    return m
+
+
+def run_both(torch, m, oracle_mod, w, **kw):
+    pp = m.FFPP.for_workload(w, **kw)
+    raw = torch.from_numpy(w.raw).cuda()
+    out = pp.run(raw, w.N_per_frame, w.frame_dims)
+    torch.cuda.synchronize()
+    ref = oracle_mod.run(w.params, w.raw, w.N_per_frame, w.frame_dims)
+    return pp, out, ref
+
+
+def test_handle_constants_equal_the_oracles(torch_cuda, ffpp_mod, oracle_mod):
+    for conf, sigma in ((0.25, 2.0), (0.2, 2.5), (0.15, 3.0)):
+        p = dict(dtype="fp16", conf_thresh=conf, iou_thresh=0.5, top_k=100, sigma_cells=sigma)
+        pp = ffpp_mod.FFPP(p, max_frames=1, max_total_candidates=8400, max_frame_w=640, max_frame_h=640)
+        info = pp.info()
+        R, w = oracle_mod.taps(sigma, 3.0)
+        assert info.radius == R
+        assert np.float32(info.logit_threshold) == np.float32(oracle_mod.logit_threshold(conf))
+        assert np.array_equal(np.array(info.taps[:2 * R + 1], dtype=np.float32), w.astype(np.float32))
+        pp.close()
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_config1_fp32(torch_cuda, ffpp_mod, oracle_mod, gen_mod, seed):
+    w = gen_mod.make_config(1, seed_offset=seed)
+    pp, out, ref = run_both(torch_cuda, ffpp_mod, oracle_mod, w)
+    assert pp.info().key_bits == 64
+    compare(out, ref, w, check_stage=pp)
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_config2_fp16(torch_cuda, ffpp_mod, oracle_mod, gen_mod, seed):
+    w = gen_mod.make_config(2, seed_offset=seed)
+    pp, out, ref = run_both(torch_cuda, ffpp_mod, oracle_mod, w)
+    assert pp.info().key_bits == 32
+    compare(out, ref, w, check_stage=pp)
+
+
+@pytest.mark.parametrize("c,B", [(3, 4), (4, 3), (5, 8)])
+def test_larger_configs_reduced_batch(torch_cuda, ffpp_mod, oracle_mod, gen_mod, c, B):
+    w = gen_mod.make_config(c, B=B)
+    pp, out, ref = run_both(torch_cuda, ffpp_mod, oracle_mod, w)
+    compare(out, ref, w, check_stage=pp)
+
+
+def test_determinism_and_reuse_of_a_handle(torch_cuda, ffpp_mod, oracle_mod, gen_mod):
+    torch = torch_cuda
+    w = gen_mod.make_config(2, B=4)
+    pp = ffpp_mod.FFPP.for_workload(w)
+    raw = torch.from_numpy(w.raw).cuda()
+    outs = []
+    for _ in range(3):
+        o = pp.run(raw, w.N_per_frame, w.frame_dims)
+        torch.cuda.synchronize()
+        outs.append((o.counts_numpy().copy(), o.boxes_numpy().copy(), o.density_numpy().copy()))
+    ref = oracle_mod.run(w.params, w.raw, w.N_per_frame, w.frame_dims)
+    for c, b, d in outs[1:]:
+        assert np.array_equal(c, outs[0][0]) and d.tobytes() == outs[0][2].tobytes()
+        for f in range(w.B):
+            assert b[f, :c[f]].tobytes() == outs[0][1][f, :c[f]].tobytes()
+    # a different geometry through the same handle, then back
+    w1 = gen_mod.make_config(2, B=1, seed_offset=5)
+    o1 = pp.run(torch.from_numpy(w1.raw).cuda(), w1.N_per_frame, w1.frame_dims)
+    torch.cuda.synchronize()
+    compare(o1, oracle_mod.run(w1.params, w1.raw, w1.N_per_frame, w1.frame_dims), w1)
+    o = pp.run(raw, w.N_per_frame, w.frame_dims)
+    torch.cuda.synchronize()
+    compare(o, ref, w)
+
+
+def test_host_buffer_entry_point(torch_cuda, ffpp_mod, oracle_mod, gen_mod):
+    w = gen_mod.make_config(5, B=4)
+    pp = ffpp_mod.FFPP.for_workload(w)
+    out = pp.run_host(w.raw, w.N_per_frame, w.frame_dims)
+    compare(out, oracle_mod.run(w.params, w.raw, w.N_per_frame, w.frame_dims), w)
