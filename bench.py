@@ -1,0 +1,372 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the libffpp hot path on the synthetic flock workloads (BASELINE.json metric:
+post-processed frames/s and candidates/s at 1 B200; % of roofline per stage).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference]
+
+One "step" = one ffpp_run over one whole batch of the chosen config (all §8(a) rows a0-a6, five kernel
+launches on one stream).  Default workload: config 5 (ragged 256-frame multi-zone batch, 6 639 360 candidates,
+66.4 MB fp16), the largest single-GPU configuration and the only one that exercises the ragged scheduler.
+Rank r of N generates its own batch (seed offset r): frames are independent, so N GPUs = N x the frames, no
+data-path collective ("scaling": "weak").
+
+Timing: every timed step is bracketed by CUDA events on the launching stream; L2 (126 MB) is flushed between
+steps by writing a 512 MB scratch buffer outside the event pair; the K step times are summed, the sum is
+max-reduced over ranks, and the whole timed loop sits between barrier + torch.cuda.synchronize() on both sides.
+`e2e` is the same metric through ffpp_run_host with pinned HOST buffers (H2D of the raw head output and D2H of
+counts, density and kept boxes inside the timed region).  `--impl reference` times the CPU oracle (oracle/) on
+a bounded sample; it is the only place besides `cpu_baseline` where bench.py executes oracle/.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "post-processed frames/sec"
+UNIT = "frames/s"
+
+CONFIG_DESC = {
+    1: "config1: B=1 640x640 fp32 [1,8400,5]",
+    2: "config2: B=16 640x640 fp16 [16,8400,5]",
+    3: "config3: B=32 1280x1280 fp16 [32,33600,5]",
+    4: "config4: B=64 1920x1088 fp16 [64,42840,5]",
+    5: "config5: ragged B=256 (64 each 640x640/1280x1280/1920x1088/1280x720, interleaved) fp16, 6639360 candidates",
+}
+
+
+def load_peaks():
+    """Roofline denominators: driver-measured MEASURED_PEAKS.json, else the profiling guide's fallback."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            p = json.load(fh)
+        return float(p["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)", float(p.get("sm_max_mhz", 1965.0))
+    return 6650.0, "fallback (B200_PROFILING.md)", 1965.0
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            parts = [x.strip() for x in ln.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1])); power.append(float(parts[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def dist_env():
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+
+
+def pair_count(n_sorted: np.ndarray) -> int:
+    n = n_sorted.astype(np.int64)
+    return int((n * (n - 1) // 2).sum())
+
+
+# --------------------------------------------------------------------------------------------------------------
+# reference arm: the oracle as it stands, on the host cores
+# --------------------------------------------------------------------------------------------------------------
+REF_SAMPLE_FRAMES = {1: 1, 2: 16, 3: 16, 4: 8, 5: 16}    # frames per reference "step" (bounded sample)
+CPU_BASELINE_FRAMES = {1: 1, 2: 16, 3: 32, 4: 48, 5: 128}  # cpu_baseline sample of the default arm (~10-30 s)
+
+
+def oracle_time(w, n_frames: int, reps: int = 1):
+    """Seconds for the oracle over the first n_frames frames of workload w (single thread, as it stands)."""
+    import oracle
+    n_frames = min(n_frames, w.B)
+    rows = int(w.N_per_frame[:n_frames].sum())
+    raw = w.raw[:rows]
+    best = None
+    for _ in range(reps):
+        t0 = time.perf_counter()
+        oracle.run(w.params, raw, w.N_per_frame[:n_frames], w.frame_dims[:n_frames])
+        dt = time.perf_counter() - t0
+        best = dt if best is None else min(best, dt)
+    return best, n_frames, rows
+
+
+def run_reference(args):
+    rank, _, world = dist_env()
+    if rank != 0:
+        return 0
+    import flockgen
+    import oracle
+    oracle.build()
+    w = flockgen.make_config(args.config)
+    nf = min(REF_SAMPLE_FRAMES[args.config], w.B)
+    rows = int(w.N_per_frame[:nf].sum())
+    for _ in range(args.warmup):
+        oracle_time(w, nf)
+    t = 0.0
+    for _ in range(args.steps):
+        t += oracle_time(w, nf)[0]
+    fps = nf * args.steps / t
+    sample = f"first {nf} of {w.B} frames of {w.name} per step ({rows} candidates), single thread"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": fps, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": CONFIG_DESC[args.config], "sample": sample},
+        "candidates_per_s": rows * args.steps / t,
+        "cpu_baseline": {"value": fps, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": fps, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# --------------------------------------------------------------------------------------------------------------
+# our arm
+# --------------------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import flockgen
+    import paper_2512_07009_b200 as ffpp
+
+    rank, local_rank, world = dist_env()
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    ffpp.load_library()
+    hbm_peak, peak_src, sm_max_mhz = load_peaks()
+
+    c = args.config
+    w = flockgen.make_config(c, seed_offset=rank)
+    B, total_cand = w.B, w.total_candidates
+    pp = ffpp.FFPP.for_workload(w)
+    info = pp.info()
+    stream = torch.cuda.current_stream()
+    raw_pinned = torch.from_numpy(w.raw).pin_memory()
+    raw_dev = raw_pinned.cuda(non_blocking=False)
+    out = pp.alloc_outputs(B, w.frame_dims)
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+
+    def step_device():
+        pp.run(raw_dev, w.N_per_frame, w.frame_dims, out=out, stream=stream)
+
+    # ---- warm-up ----
+    for _ in range(max(args.warmup, 3)):
+        flush.zero_()
+        step_device()
+    torch.cuda.synchronize()
+    n_sorted = pp.debug_read(1, B)
+    n_surv = pp.debug_read(0, B)
+    kept = out.counts_numpy().astype(np.int64)
+    pairs = pair_count(n_sorted)
+
+    # ---- timed: device-resident inputs ----
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    sampler = ClockSampler(local_rank)
+    barrier(); torch.cuda.synchronize()
+    sampler.start()
+    t_wall0 = time.perf_counter()
+    for k in range(args.steps):
+        flush.zero_()
+        ev[k][0].record(stream)
+        step_device()
+        ev[k][1].record(stream)
+    torch.cuda.synchronize(); barrier()
+    t_wall = time.perf_counter() - t_wall0
+    step_ms = np.array([a.elapsed_time(b) for a, b in ev], dtype=np.float64)
+    total_ms = float(step_ms.sum())
+
+    # ---- per-stage durations (library's own events on the launching stream), cold L2, same launch configuration ----
+    pp.set_stage_timing(True)
+    stage = []
+    for _ in range(min(max(args.steps, 3), 20)):
+        flush.zero_()
+        step_device()
+        torch.cuda.synchronize()
+        stage.append(pp.stage_ms().astype(np.float64))
+    pp.set_stage_timing(False)
+    stage_ms = np.mean(np.stack(stage), axis=0)
+
+    # ---- e2e: host buffers through ffpp_run_host ----
+    cells = int(out.density_offsets[-1])
+    h_boxes = torch.empty((B, pp.top_k, 6), dtype=torch.float32).pin_memory()
+    h_counts = torch.empty((B,), dtype=torch.int32).pin_memory()
+    h_density = torch.empty((cells,), dtype=torch.float32).pin_memory()
+    hout = ffpp.Output()
+    hout.boxes, hout.counts, hout.density, hout.density_offsets = h_boxes, h_counts, h_density, out.density_offsets
+
+    def step_host():
+        pp.run_host(raw_pinned, w.N_per_frame, w.frame_dims, out=hout, stream=stream)
+
+    e2e_steps = args.steps
+    for _ in range(3):
+        step_host()
+    barrier(); torch.cuda.synchronize()
+    t_e2e = 0.0
+    for _ in range(e2e_steps):
+        flush.zero_(); torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        step_host()
+        t_e2e += time.perf_counter() - t0
+    torch.cuda.synchronize(); barrier()
+    clocks = sampler.stop()
+    h2d = int(w.raw.nbytes)
+    d2h = int(4 * B + 4 * cells + 24 * int(kept.sum()))
+
+    # ---- reduce over ranks ----
+    if world > 1:
+        t = torch.tensor([total_ms, t_e2e], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms, t_e2e = float(t[0]), float(t[1])
+        u = torch.tensor([B, total_cand], dtype=torch.float64, device="cuda")
+        dist.all_reduce(u, op=dist.ReduceOp.SUM)
+        frames_all, cand_all = float(u[0]), float(u[1])
+    else:
+        frames_all, cand_all = float(B), float(total_cand)
+
+    if rank == 0:
+        K = args.steps
+        fps = frames_all * K / (total_ms * 1e-3)
+        cps = cand_all * K / (total_ms * 1e-3)
+        elem = 2 if w.params["dtype"] == "fp16" else 4
+        key_b = info.key_bits // 8
+        cell_b = 4 * cells
+        kept_n = int(kept.sum())
+        # algorithmic bytes / ops per launch
+        a1_bytes = total_cand * 5 * elem + int(n_surv.sum()) * key_b
+        a56_bytes = cell_b + 16 * kept_n
+        stages = {}
+        names = ffpp.STAGE_NAMES
+        for i, nm in enumerate(names):
+            stages[nm] = {"ms": float(stage_ms[i])}
+        s1 = stages["a1_threshold_compact"]; s1["algorithmic_bytes"] = a1_bytes
+        s1["GB/s"] = a1_bytes / (stage_ms[1] * 1e-3) / 1e9; s1["frac_of_hbm_peak"] = s1["GB/s"] / hbm_peak
+        s5 = stages["a5a6_density"]; s5["algorithmic_bytes"] = a56_bytes
+        s5["GB/s"] = a56_bytes / (stage_ms[5] * 1e-3) / 1e9; s5["frac_of_hbm_peak"] = s5["GB/s"] / hbm_peak
+        s3 = stages["a3_nms_mask"]; s3["iou_pairs"] = pairs
+        s3["Gpairs/s"] = pairs / (stage_ms[3] * 1e-3) / 1e9
+        # dominant kernel = the stage with the largest share of the step
+        dom = int(np.argmax(stage_ms[1:])) + 1
+        alu_peak_gpairs = 148 * 128 * sm_max_mhz * 1e6 / ffpp.NMS_ALU_OPS_PER_PAIR / 1e9
+        if dom == 3:
+            roofline = {"kernel": "k3_nms_mask", "bound": "alu", "achieved": s3["Gpairs/s"], "peak": alu_peak_gpairs,
+                        "unit": "Gpair/s", "frac": s3["Gpairs/s"] / alu_peak_gpairs, "traffic": None,
+                        "peak_source": f"148 SM x 128 fp32 lanes x {sm_max_mhz:.0f} MHz / {ffpp.NMS_ALU_OPS_PER_PAIR} ALU ops per IoU pair "
+                                       "(DESIGN.md §Kernels a3)"}
+        else:
+            sd = stages[names[dom]]
+            ab = sd.get("algorithmic_bytes")
+            roofline = {"kernel": names[dom], "bound": "hbm", "achieved": sd.get("GB/s"), "peak": hbm_peak, "unit": "GB/s",
+                        "frac": (sd.get("GB/s") / hbm_peak) if ab else None, "traffic": None, "peak_source": peak_src}
+        roofline["hbm_peak_source"] = peak_src
+        tr_path = os.path.join(ROOT, "profiles", f"traffic_config{c}.json")
+        if os.path.exists(tr_path):      # dram bytes per launch from the committed ncu --set full capture
+            with open(tr_path) as fh:
+                roofline["traffic"] = json.load(fh).get(roofline["kernel"])
+
+        # ---- CPU baseline: the oracle as it stands on this box's host cores, bounded sample ----
+        cpu = None
+        if world == 1 or True:
+            try:
+                t_cpu, nf, rows = oracle_time(w, CPU_BASELINE_FRAMES[c])
+                cpu = {"value": nf / t_cpu, "unit": UNIT, "cores": 1, "kind": "oracle",
+                       "sample": f"first {nf} of {B} frames of {w.name} ({rows} candidates), one pass, single thread, {t_cpu:.2f} s",
+                       "candidates_per_s": rows / t_cpu, "host_cpus": os.cpu_count()}
+            except Exception as exc:  # the baseline is reported, never required for the GPU numbers
+                cpu = {"value": None, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": f"failed: {exc}"}
+
+        line = {
+            "metric": METRIC, "value": fps, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
+            "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": CONFIG_DESC[c], "frames_per_step_per_gpu": B, "candidates_per_step_per_gpu": total_cand,
+                       "input_dtype": w.params["dtype"], "top_k": w.params["top_k"], "conf": w.params["conf_thresh"],
+                       "iou": w.params["iou_thresh"], "sigma_cells": w.params["sigma_cells"],
+                       "l2": "flushed between steps (512 MB write outside the event pair)", "seed": "config_seed(c)+rank"},
+            "candidates_per_s": cps,
+            "step_ms_min": float(step_ms.min()), "step_ms_median": float(np.median(step_ms)), "wall_s_timed_loop": t_wall,
+            "e2e": {"value": frames_all * e2e_steps / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "ms_per_step": 1e3 * t_e2e / e2e_steps, "candidates_per_s": cand_all * e2e_steps / t_e2e,
+                    "api": "ffpp_run_host (pinned host buffers, copies + sync inside the timed region)"},
+            "gpu_launches": 5 * K,
+            "roofline": roofline,
+            "stages": stages,
+            "cpu_baseline": cpu,
+            "clocks": clocks,
+            "workload_stats": {"survivors": int(n_surv.sum()), "entering_nms": int(n_sorted.sum()), "kept": kept_n,
+                               "iou_pairs": pairs, "density_cells": cells, "workspace_bytes": int(info.workspace_bytes)},
+            "paper_context": "paper: up to 2x pipeline speedup on AWS g4dn.2xlarge (T4), $0.69 -> $0.31 per run; no number for this path",
+        }
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -31,6 +31,10 @@ FFPP_OK, FFPP_EINVAL, FFPP_ECAPACITY, FFPP_ECUDA, FFPP_ENOMEM = 0, -1, -2, -3, -
 NUM_STAGES = 6
 STAGE_NAMES = ["a0_schedule", "a1_threshold_compact", "a2_sort_topk_decode", "a3_nms_mask", "a4_nms_sweep", "a5a6_density"]
 
+# ALU ops per IoU pair that any all-pairs bitmask NMS must issue: the four chained compare-and-AND of the strict
+# overlap test (DESIGN.md §Kernels a3).  bench.py divides the fp32 lane rate by this to get the pairs/s ceiling.
+NMS_ALU_OPS_PER_PAIR = 4
+
 BOX_DTYPE = np.dtype([("x1", "<f4"), ("y1", "<f4"), ("x2", "<f4"), ("y2", "<f4"), ("score", "<f4"), ("cand_index", "<i4")])
 
 EXPORTS = ["ffpp_create", "ffpp_run", "ffpp_run_host", "ffpp_destroy", "ffpp_last_error", "ffpp_get_info",
