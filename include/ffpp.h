@@ -52,8 +52,13 @@ typedef struct ffpp_params {
   int32_t max_frame_w;     /* capacity: W_f <= max_frame_w                                                          */
   int32_t max_frame_h;     /* capacity: H_f <= max_frame_h                                                          */
   int64_t max_total_cells; /* capacity: sum_f (W_f/cell)(H_f/cell); 0 = max_frames * (max_w/cell)(max_h/cell)       */
-  int64_t nms_workspace_bytes; /* capacity of the suppression-mask workspace; 0 = worst case for max_frames frames
-                                  of min(top_k, max candidates of a max_w x max_h frame) boxes                      */
+  int64_t nms_workspace_bytes; /* capacity of the NMS suppression-word workspace; 0 = default: tiled mode
+                                  nms_slots_per_block slots per 32-box block, dense mode the worst case for
+                                  max_frames frames of min(top_k, max candidates of a max_w x max_h frame) boxes   */
+  int32_t nms_mode;        /* 0 = spatially tiled suppression words (default); 1 = dense rank-order 64x64 bitmask
+                              + single-warp sweep.  Both compute the same greedy NMS (O5)           */
+  int32_t nms_slots_per_block; /* tiled mode: suppression-word slots (192 B each) reserved per 32-box block;
+                                  0 = 64.  A block that needs more falls back to recomputing its words            */
 } ffpp_params;
 
 /* One kept detection (24 bytes).  score = sigmoid(logit) in fp32; cand_index = candidate index within its frame. */

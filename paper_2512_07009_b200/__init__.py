@@ -21,7 +21,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 _LIB = os.path.join(_HERE, "libffpp.so")
-_SOURCES = ["ffpp.cu", "ffpp_kernels.cuh", "ffpp_common.cuh"]
+_SOURCES = ["ffpp.cu", "ffpp_kernels.cuh", "ffpp_nms_dense.cuh", "ffpp_common.cuh"]
 _INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
@@ -49,6 +49,7 @@ class FFPPParams(ctypes.Structure):
         ("max_frames", ctypes.c_int32), ("max_total_candidates", ctypes.c_int64),
         ("max_frame_w", ctypes.c_int32), ("max_frame_h", ctypes.c_int32),
         ("max_total_cells", ctypes.c_int64), ("nms_workspace_bytes", ctypes.c_int64),
+        ("nms_mode", ctypes.c_int32), ("nms_slots_per_block", ctypes.c_int32),
     ]
 
 
@@ -108,7 +109,8 @@ def load_library() -> ctypes.CDLL:
 
 
 def make_params(params: dict, *, max_frames: int, max_total_candidates: int, max_frame_w: int, max_frame_h: int,
-                max_total_cells: int = 0, nms_workspace_bytes: int = 0) -> FFPPParams:
+                max_total_cells: int = 0, nms_workspace_bytes: int = 0, nms_mode: int = 0,
+                nms_slots_per_block: int = 0) -> FFPPParams:
     p = FFPPParams()
     p.dtype = 1 if params["dtype"] == "fp16" else 0
     p.conf_thresh = params["conf_thresh"]
@@ -126,6 +128,8 @@ def make_params(params: dict, *, max_frames: int, max_total_candidates: int, max
     p.max_frame_w, p.max_frame_h = max_frame_w, max_frame_h
     p.max_total_cells = max_total_cells
     p.nms_workspace_bytes = nms_workspace_bytes
+    p.nms_mode = nms_mode
+    p.nms_slots_per_block = nms_slots_per_block
     return p
 
 
@@ -149,7 +153,7 @@ class FFPP:
     """One libffpp handle (ffpp_create / ffpp_destroy) on the current CUDA device."""
 
     def __init__(self, params: dict, *, max_frames: int, max_total_candidates: int, max_frame_w: int, max_frame_h: int,
-                 max_total_cells: int = 0, nms_workspace_bytes: int = 0):
+                 max_total_cells: int = 0, nms_workspace_bytes: int = 0, nms_mode: int = 0, nms_slots_per_block: int = 0):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2512_07009_b200 needs a CUDA sm_100 device; there is no CPU fallback")
@@ -163,7 +167,8 @@ class FFPP:
         self._torch_dtype = torch.float16 if params["dtype"] == "fp16" else torch.float32
         self._p = make_params(params, max_frames=max_frames, max_total_candidates=max_total_candidates,
                               max_frame_w=max_frame_w, max_frame_h=max_frame_h, max_total_cells=max_total_cells,
-                              nms_workspace_bytes=nms_workspace_bytes)
+                              nms_workspace_bytes=nms_workspace_bytes, nms_mode=nms_mode,
+                              nms_slots_per_block=nms_slots_per_block)
         self._h = ctypes.c_void_p()
         rc = self._lib.ffpp_create(ctypes.byref(self._p), ctypes.byref(self._h))
         if rc != FFPP_OK:

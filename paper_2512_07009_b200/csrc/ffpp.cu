@@ -9,6 +9,7 @@
 #include <vector>
 
 #include "ffpp_kernels.cuh"
+#include "ffpp_nms_dense.cuh"
 
 using namespace ffpp;
 
@@ -17,7 +18,7 @@ namespace {
 thread_local std::string g_create_error;
 
 struct DeviceMeta {           // one pinned block + one device block, uploaded with a single copy
-  size_t frames_off, cand_off_off, unit_prefix_off, tile_prefix_off, bytes;
+  size_t frames_off, cand_off_off, unit_prefix_off, bytes;
 };
 
 DeviceMeta meta_layout(int max_frames) {
@@ -27,7 +28,6 @@ DeviceMeta meta_layout(int max_frames) {
   o = (o + 15) & ~(size_t)15;
   m.cand_off_off = o; o += sizeof(int64_t) * ((size_t)max_frames + 1);
   m.unit_prefix_off = o; o += sizeof(int32_t) * ((size_t)max_frames + 1);
-  m.tile_prefix_off = o; o += sizeof(int32_t) * ((size_t)max_frames + 1);
   m.bytes = (o + 15) & ~(size_t)15;
   return m;
 }
@@ -38,20 +38,34 @@ struct ffpp_handle {
   ffpp_params p;
   Consts cst;
   bool half = false;
+  bool dense = false;                 // nms_mode == 1
   int key_bytes = 8;
+  int key_slots = 0;                  // a2: keys staged in shared memory
+  int nb32cap = 0;                    // ceil(top_k / 32): stride of the per-block arrays
   int sm_count = 148;
   int max_frame_cand = 0;
   int64_t max_total_cells = 0;
-  int64_t mask_words_cap = 0;
+  int64_t mask_words_cap = 0;         // dense mode: uint64 words
+  int64_t slot_cap_total = 0;         // tiled mode: suppression-word slots (32 words each)
   std::string err;
 
   // device workspace
   uint8_t* d_meta = nullptr;
   void* d_surv_keys = nullptr;
-  int* d_counters = nullptr;          // [0,max_frames) survivor counts | [max_frames, 2*max_frames) sorted counts
+  int* d_counters = nullptr;          // 4 x max_frames: survivor counts | sorted counts | slot counters | frame_err
   float4* d_sorted_box = nullptr;
   float* d_sorted_logit = nullptr;
   int* d_sorted_idx = nullptr;
+  uint32_t* d_hist32 = nullptr;       // a5: uint16 count per density cell, two per word
+  // tiled NMS
+  float4* d_sp_box = nullptr;
+  uint16_t* d_sp_rank = nullptr;
+  float4* d_bbox32 = nullptr;
+  int* d_slot_base = nullptr;
+  uint16_t* d_nzc = nullptr;
+  uint32_t* d_W32 = nullptr;
+  uint16_t* d_WQ = nullptr;
+  // dense NMS
   unsigned long long* d_mask = nullptr;
   int64_t workspace_bytes = 0;
   // pinned staging for the descriptor table
@@ -61,7 +75,7 @@ struct ffpp_handle {
   // geometry of the last batch (skip rebuild + upload when unchanged)
   int last_B = -1;
   std::vector<int32_t> last_N, last_dims;
-  int total_units = 0, total_tiles = 0;
+  int total_units = 0, max_tiles = 0, max_nmax = 0;
   int64_t total_cand = 0, total_cells = 0;
   // host-buffer path staging (allocated on first ffpp_run_host)
   void* d_in = nullptr;
@@ -75,6 +89,8 @@ struct ffpp_handle {
 
   int* surv_cnt() const { return d_counters; }
   int* n_sorted() const { return d_counters + p.max_frames; }
+  int* slot_ctr() const { return d_counters + 2 * (size_t)p.max_frames; }
+  int* frame_err() const { return d_counters + 3 * (size_t)p.max_frames; }
 };
 
 namespace {
@@ -115,10 +131,10 @@ int schedule(ffpp_handle* h, int B, const int32_t* N, const int32_t* dims, cudaS
   FrameDesc* fr = reinterpret_cast<FrameDesc*>(h->h_meta + h->ml.frames_off);
   int64_t* coff = reinterpret_cast<int64_t*>(h->h_meta + h->ml.cand_off_off);
   int32_t* uoff = reinterpret_cast<int32_t*>(h->h_meta + h->ml.unit_prefix_off);
-  int32_t* toff = reinterpret_cast<int32_t*>(h->h_meta + h->ml.tile_prefix_off);
   const int smax = p.strides[p.num_levels - 1];
   const int R = h->cst.radius;
-  int64_t cand = 0, cells = 0, mwords = 0, units = 0, tiles = 0;
+  int64_t cand = 0, cells = 0, mwords = 0, units = 0, slots = 0;
+  int max_tiles = 0, max_nmax = 0;
   for (int f = 0; f < B; ++f) {
     const int W = dims[2 * f], H = dims[2 * f + 1];
     if (W <= 0 || H <= 0) return fail(h, FFPP_EINVAL, "frame_dims: W and H must be positive");
@@ -140,28 +156,45 @@ int schedule(ffpp_handle* h, int B, const int32_t* N, const int32_t* dims, cudaS
     if (n > (1 << 20)) return fail(h, FFPP_ECAPACITY, "frame has more than 2^20 candidates");
     d.cand_off = cand; d.N = (int32_t)n; d.W = W; d.H = H;
     d.nmax = (int32_t)(n < p.top_k ? n : p.top_k);
-    d.nbmax = (d.nmax + kNmsTile - 1) / kNmsTile;
-    d.mask_off = mwords;
     d.dens_off = cells;
     d.gw = W / p.cell_px; d.gh = H / p.cell_px;
     if (d.gw < R || d.gh < R) return fail(h, FFPP_EINVAL, "density grid smaller than the Gaussian radius");
-    d.tiles_x = (d.gw + K5_TW - 1) / K5_TW; d.tiles_y = (d.gh + K5_TH - 1) / K5_TH;
+    int hs = 0;
+    while ((256 << hs) < std::max(W, H)) ++hs;
+    d.hshift = hs;
+    if (h->dense) {
+      d.nbmax = (d.nmax + kNmsTile - 1) / kNmsTile;
+      d.mask_off = mwords;
+      mwords += mask_words(d.nbmax);
+      uoff[f] = (int32_t)units;
+      units += k3d_units(d.nbmax);
+      if (units > 0x7fffffff) return fail(h, FFPP_ECAPACITY, "work list too large");
+    } else {
+      const int64_t nb = (d.nmax + kBlk - 1) / kBlk;
+      d.slot_off = slots;
+      d.slot_cap = (int32_t)std::min<int64_t>(nb * nb, nb * h->p.nms_slots_per_block);
+      slots += d.slot_cap;
+      uoff[f] = 0;
+    }
     fr[f] = d;
-    coff[f] = cand; uoff[f] = (int32_t)units; toff[f] = (int32_t)tiles;
-    cand += n; cells += (int64_t)d.gw * d.gh; mwords += mask_words(d.nbmax);
-    units += k3_units(d.nbmax); tiles += (int64_t)d.tiles_x * d.tiles_y;
-    if (units > 0x7fffffff || tiles > 0x7fffffff) return fail(h, FFPP_ECAPACITY, "work list too large");
+    coff[f] = cand;
+    cand += n; cells += (int64_t)d.gw * d.gh;
+    const int tiles = ((d.gw + K5_TW - 1) / K5_TW) * ((d.gh + K5_TH - 1) / K5_TH);
+    max_tiles = std::max(max_tiles, tiles);
+    max_nmax = std::max(max_nmax, (int)d.nmax);
   }
-  coff[B] = cand; uoff[B] = (int32_t)units; toff[B] = (int32_t)tiles;
+  coff[B] = cand; uoff[B] = (int32_t)units;
   if (cand > p.max_total_candidates) return fail(h, FFPP_ECAPACITY, "sum N_f exceeds max_total_candidates");
   if (cells > h->max_total_cells) return fail(h, FFPP_ECAPACITY, "density cells exceed max_total_cells");
   if (mwords > h->mask_words_cap) return fail(h, FFPP_ECAPACITY, "suppression mask exceeds nms_workspace_bytes");
+  if (slots > h->slot_cap_total) return fail(h, FFPP_ECAPACITY, "suppression-word pool exceeds nms_workspace_bytes");
   FFPP_CUDA(h, cudaMemcpyAsync(h->d_meta, h->h_meta, h->ml.bytes, cudaMemcpyHostToDevice, stream));
   FFPP_CUDA(h, cudaEventRecord(h->meta_done, stream));
   h->last_B = B;
   h->last_N.assign(N, N + B);
   h->last_dims.assign(dims, dims + 2 * B);
-  h->total_units = (int)units; h->total_tiles = (int)tiles; h->total_cand = cand; h->total_cells = cells;
+  h->total_units = (int)units; h->max_tiles = max_tiles; h->max_nmax = max_nmax;
+  h->total_cand = cand; h->total_cells = cells;
   return FFPP_OK;
 }
 
@@ -171,7 +204,6 @@ int launch_all(ffpp_handle* h, const void* raw, int B, cudaStream_t st, ffpp_box
   const FrameDesc* frames = reinterpret_cast<const FrameDesc*>(h->d_meta + h->ml.frames_off);
   const int64_t* coff = reinterpret_cast<const int64_t*>(h->d_meta + h->ml.cand_off_off);
   const int32_t* uoff = reinterpret_cast<const int32_t*>(h->d_meta + h->ml.unit_prefix_off);
-  const int32_t* toff = reinterpret_cast<const int32_t*>(h->d_meta + h->ml.tile_prefix_off);
   const Consts& c = h->cst;
   const bool tm = h->timing;
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[1], st));
@@ -180,39 +212,44 @@ int launch_all(ffpp_handle* h, const void* raw, int B, cudaStream_t st, ffpp_box
   {
     const int64_t row = kHalf ? 10 : 20;
     const int64_t nchunks = (h->total_cand * row + K1_CHUNK_BYTES - 1) / K1_CHUNK_BYTES;
-    int64_t grid = (int64_t)h->sm_count * 3;
+    int64_t grid = (int64_t)h->sm_count * K1_CTAS_PER_SM;
     if (grid > nchunks) grid = nchunks;
     k1_threshold_compact<kHalf, KeyT><<<(unsigned)grid, K1_THREADS, K1_STAGES * K1_CHUNK_BYTES, st>>>(
         static_cast<const uint8_t*>(raw), h->total_cand, B, coff, c.logit_thr, static_cast<KeyT*>(h->d_surv_keys),
         h->surv_cnt());
   }
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[2], st));
-  // a2
-  {
-    const int cap = h->p.top_k;
-    const size_t smem = 2 * (size_t)cap * sizeof(KeyT) + K2_WARPS * 256 * sizeof(uint16_t) + 256 * sizeof(uint32_t) + sizeof(K2Misc);
-    k2_sort_topk_decode<kHalf, KeyT><<<B, K2_THREADS, smem, st>>>(static_cast<const uint8_t*>(raw), frames,
-                                                                   static_cast<const KeyT*>(h->d_surv_keys), h->surv_cnt(), c,
-                                                                   cap, h->d_sorted_box, h->d_sorted_logit, h->d_sorted_idx,
-                                                                   h->n_sorted());
-  }
+  // a2 (+ clears the a5 histogram)
+  k2_sort_topk_decode<kHalf, KeyT><<<B, K2_THREADS, k2_smem_bytes((size_t)h->key_slots, sizeof(KeyT)), st>>>(
+      static_cast<const uint8_t*>(raw), frames, static_cast<const KeyT*>(h->d_surv_keys), h->surv_cnt(), c, h->key_slots,
+      h->nb32cap, h->d_sorted_box, h->d_sorted_logit, h->d_sorted_idx, h->n_sorted(), h->d_sp_box, h->d_sp_rank,
+      h->d_bbox32, h->d_hist32, h->dense ? 0 : 1);
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[3], st));
-  // a3
-  if (h->total_units > 0)
-    k3_nms_mask<<<h->total_units, K3_THREADS, 0, st>>>(frames, uoff, B, h->d_sorted_box, h->n_sorted(), c, h->d_mask);
-  if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[4], st));
-  // a4
-  {
+  if (h->dense) {
+    // a3 / a4, dense rank-order bitmask
+    if (h->total_units > 0)
+      k3d_nms_mask<<<h->total_units, K3D_THREADS, 0, st>>>(frames, uoff, B, h->d_sorted_box, h->n_sorted(), c, h->d_mask);
+    if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[4], st));
     const size_t smem = sizeof(unsigned long long) * (size_t)((h->p.top_k + kNmsTile - 1) / kNmsTile);
-    k4_nms_sweep<<<B, K4_THREADS, smem, st>>>(frames, h->d_sorted_box, h->d_sorted_logit, h->d_sorted_idx, h->n_sorted(), c,
-                                              h->d_mask, out_boxes, out_counts);
+    k4d_nms_sweep<<<B, K4D_THREADS, smem, st>>>(frames, h->d_sorted_box, h->d_sorted_logit, h->d_sorted_idx, h->n_sorted(),
+                                                c, h->d_mask, out_boxes, out_counts, h->d_hist32);
+  } else {
+    // a3 / a4, spatially tiled
+    const dim3 g3((unsigned)((h->max_nmax + K3_THREADS - 1) / K3_THREADS), (unsigned)B);
+    if (g3.x > 0)
+      k3_nms_tiles<<<g3, K3_THREADS, 0, st>>>(frames, h->n_sorted(), h->d_sp_box, h->d_sp_rank, h->d_bbox32, c, h->nb32cap,
+                                              h->slot_ctr(), h->d_slot_base, h->d_nzc, h->d_W32, h->d_WQ, h->frame_err());
+    if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[4], st));
+    k4_resolve_emit<<<B, K4_THREADS, 0, st>>>(frames, h->n_sorted(), h->d_sorted_box, h->d_sorted_logit, h->d_sorted_idx,
+                                              h->d_sp_rank, h->d_nzc, h->d_slot_base, h->d_W32, h->d_WQ, h->frame_err(), c,
+                                              h->nb32cap, out_boxes, out_counts, h->d_hist32);
   }
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[5], st));
-  // a5-a6
+  // a6
   {
-    const int R = c.radius;
-    const size_t smem = sizeof(int) * (size_t)(K5_TH + 2 * R) * (K5_TW + 2 * R) + sizeof(float) * (size_t)(K5_TH + 2 * R) * K5_TW;
-    k5_density<<<h->total_tiles, K5_THREADS, smem, st>>>(frames, toff, B, out_boxes, out_counts, c, out_density);
+    const dim3 g5((unsigned)h->max_tiles, (unsigned)B);
+    k5_density<<<g5, K5_THREADS, k5_smem_bytes(c.radius), st>>>(frames, c, reinterpret_cast<const uint16_t*>(h->d_hist32),
+                                                                 out_density);
   }
   if (tm) {
     FFPP_CUDA(h, cudaEventRecord(h->ev[6], st));
@@ -226,7 +263,7 @@ template <bool kHalf, typename KeyT>
 int set_kernel_attrs(ffpp_handle* h) {
   const size_t s1 = K1_STAGES * K1_CHUNK_BYTES;
   FFPP_CUDA(h, cudaFuncSetAttribute(k1_threshold_compact<kHalf, KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s1));
-  const size_t s2 = 2 * (size_t)h->p.top_k * sizeof(KeyT) + K2_WARPS * 256 * sizeof(uint16_t) + 256 * sizeof(uint32_t) + sizeof(K2Misc);
+  const size_t s2 = k2_smem_bytes((size_t)h->key_slots, sizeof(KeyT));
   FFPP_CUDA(h, cudaFuncSetAttribute(k2_sort_topk_decode<kHalf, KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s2));
   return FFPP_OK;
 }
@@ -253,15 +290,27 @@ int ffpp_create(const ffpp_params* p, ffpp_handle** out) {
   const int R = (int)std::floor((double)p->truncate_sigmas * (double)p->sigma_cells);
   if (R < 1 || R > kMaxRadius) return fail(nullptr, FFPP_EINVAL, "Gaussian radius floor(truncate*sigma) must be 1..32");
 
+  if (p->nms_mode != 0 && p->nms_mode != 1) return fail(nullptr, FFPP_EINVAL, "nms_mode must be 0 (tiled) or 1 (dense)");
+  if (p->nms_slots_per_block < 0) return fail(nullptr, FFPP_EINVAL, "nms_slots_per_block must be >= 0");
   ffpp_handle* h = new (std::nothrow) ffpp_handle();
   if (!h) return fail(nullptr, FFPP_ENOMEM, "host allocation failed");
   h->p = *p;
   h->half = p->dtype == 1;
+  h->dense = p->nms_mode == 1;
   const int64_t nmaxframe = frame_candidates(*p, p->max_frame_w, p->max_frame_h);
   h->max_frame_cand = (int)std::min<int64_t>(nmaxframe, 1 << 20);
   h->key_bytes = (h->half && nmaxframe <= 65536) ? 4 : 8;
-  const int kcap = h->key_bytes == 4 ? 24576 : 12288;
-  if (p->top_k > kcap) { delete h; return fail(nullptr, FFPP_EINVAL, "top_k exceeds the shared-memory sort capacity (24576 / 12288)"); }
+  {
+    // a2 shared-memory budget: everything the 227 KB opt-in limit leaves after the histograms holds keys
+    const size_t fixed = k2_smem_bytes(0, h->key_bytes) + 1024;      // + static shared of the kernel
+    const int64_t fit = (int64_t)((232448 - fixed) / h->key_bytes);
+    if (2 * (int64_t)p->top_k > fit || p->top_k > 24576) {
+      delete h;
+      return fail(nullptr, FFPP_EINVAL, "top_k exceeds the shared-memory sort capacity (24576 with 32-bit keys, 12288 with 64-bit keys)");
+    }
+    h->key_slots = (int)std::min<int64_t>(fit, std::max<int64_t>(2 * (int64_t)p->top_k, h->max_frame_cand));
+  }
+  h->nb32cap = (p->top_k + kBlk - 1) / kBlk;
 
   // constants
   Consts& c = h->cst;
@@ -296,8 +345,20 @@ int ffpp_create(const ffpp_params* p, ffpp_handle** out) {
   // capacities
   const int64_t cells_frame = (int64_t)(p->max_frame_w / p->cell_px) * (p->max_frame_h / p->cell_px);
   h->max_total_cells = p->max_total_cells > 0 ? p->max_total_cells : cells_frame * p->max_frames;
-  const int nbcap = (int)((std::min<int64_t>(p->top_k, nmaxframe) + kNmsTile - 1) / kNmsTile);
-  h->mask_words_cap = p->nms_workspace_bytes > 0 ? p->nms_workspace_bytes / 8 : mask_words(nbcap) * p->max_frames;
+  const int64_t nmax_cap = std::min<int64_t>(p->top_k, nmaxframe);
+  if (h->dense) {
+    const int nbcap = (int)((nmax_cap + kNmsTile - 1) / kNmsTile);
+    h->mask_words_cap = p->nms_workspace_bytes > 0 ? p->nms_workspace_bytes / 8 : mask_words(nbcap) * p->max_frames;
+  } else {
+    const int64_t nb = (nmax_cap + kBlk - 1) / kBlk;
+    const int64_t slot_bytes = kBlk * (sizeof(uint32_t) + sizeof(uint16_t));
+    int64_t spb = p->nms_slots_per_block > 0 ? p->nms_slots_per_block : 64;
+    if (p->nms_workspace_bytes > 0) spb = std::max<int64_t>(1, p->nms_workspace_bytes / slot_bytes / (nb * p->max_frames));
+    spb = std::min<int64_t>(spb, nb);
+    h->p.nms_slots_per_block = (int32_t)spb;
+    h->slot_cap_total = spb * nb * p->max_frames;
+    if (h->slot_cap_total > 0x7fffffff) return bail(FFPP_EINVAL, "suppression-word pool has more than 2^31 slots");
+  }
 
   h->ml = meta_layout(p->max_frames);
   auto dalloc = [&](void** ptr, size_t bytes) {
@@ -307,13 +368,22 @@ int ffpp_create(const ffpp_params* p, ffpp_handle** out) {
     return ee;
   };
   const size_t K = (size_t)p->top_k, F = (size_t)p->max_frames;
+  const size_t pool = (size_t)h->slot_cap_total * kBlk;
   if ((e = dalloc((void**)&h->d_meta, h->ml.bytes)) != cudaSuccess ||
       (e = dalloc(&h->d_surv_keys, (size_t)p->max_total_candidates * h->key_bytes)) != cudaSuccess ||
-      (e = dalloc((void**)&h->d_counters, 2 * F * sizeof(int))) != cudaSuccess ||
+      (e = dalloc((void**)&h->d_counters, 4 * F * sizeof(int))) != cudaSuccess ||
       (e = dalloc((void**)&h->d_sorted_box, F * K * sizeof(float4))) != cudaSuccess ||
       (e = dalloc((void**)&h->d_sorted_logit, F * K * sizeof(float))) != cudaSuccess ||
       (e = dalloc((void**)&h->d_sorted_idx, F * K * sizeof(int))) != cudaSuccess ||
-      (e = dalloc((void**)&h->d_mask, (size_t)h->mask_words_cap * 8)) != cudaSuccess) {
+      (e = dalloc((void**)&h->d_hist32, ((size_t)h->max_total_cells / 2 + 2) * sizeof(uint32_t))) != cudaSuccess ||
+      (e = dalloc((void**)&h->d_mask, (size_t)h->mask_words_cap * 8)) != cudaSuccess ||
+      (!h->dense && ((e = dalloc((void**)&h->d_sp_box, F * K * sizeof(float4))) != cudaSuccess ||
+                     (e = dalloc((void**)&h->d_sp_rank, F * K * sizeof(uint16_t))) != cudaSuccess ||
+                     (e = dalloc((void**)&h->d_nzc, F * K * sizeof(uint16_t))) != cudaSuccess ||
+                     (e = dalloc((void**)&h->d_bbox32, F * (size_t)h->nb32cap * sizeof(float4))) != cudaSuccess ||
+                     (e = dalloc((void**)&h->d_slot_base, F * (size_t)h->nb32cap * sizeof(int))) != cudaSuccess ||
+                     (e = dalloc((void**)&h->d_W32, pool * sizeof(uint32_t))) != cudaSuccess ||
+                     (e = dalloc((void**)&h->d_WQ, pool * sizeof(uint16_t))) != cudaSuccess))) {
     cudaGetLastError();
     return bail(e == cudaErrorMemoryAllocation ? FFPP_ENOMEM : FFPP_ECUDA, std::string("workspace cudaMalloc: ") + cudaGetErrorString(e));
   }
@@ -327,7 +397,7 @@ int ffpp_create(const ffpp_params* p, ffpp_handle** out) {
   else rc = set_kernel_attrs<false, uint64_t>(h);
   if (rc != FFPP_OK) { std::string m = h->err; return bail(rc, m); }
   {
-    const size_t s5 = sizeof(int) * (size_t)(K5_TH + 2 * R) * (K5_TW + 2 * R) + sizeof(float) * (size_t)(K5_TH + 2 * R) * K5_TW;
+    const size_t s5 = k5_smem_bytes(R);
     if ((e = cudaFuncSetAttribute(k5_density, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s5)) != cudaSuccess)
       return bail(FFPP_ECUDA, std::string("cudaFuncSetAttribute(k5): ") + cudaGetErrorString(e));
   }
@@ -347,7 +417,7 @@ int ffpp_run(ffpp_handle* h, const void* raw, int32_t B, const int32_t* N_per_fr
   if (h->timing) FFPP_CUDA(h, cudaEventRecord(h->ev[0], st));
   int rc = schedule(h, B, N_per_frame, frame_dims, st);
   if (rc != FFPP_OK) return rc;
-  FFPP_CUDA(h, cudaMemsetAsync(h->d_counters, 0, sizeof(int) * 2 * (size_t)h->p.max_frames, st));
+  FFPP_CUDA(h, cudaMemsetAsync(h->d_counters, 0, sizeof(int) * 4 * (size_t)h->p.max_frames, st));
   if (h->half && h->key_bytes == 4) return launch_all<true, uint32_t>(h, raw, B, st, out_boxes, out_counts, out_density);
   if (h->half) return launch_all<true, uint64_t>(h, raw, B, st, out_boxes, out_counts, out_density);
   return launch_all<false, uint64_t>(h, raw, B, st, out_boxes, out_counts, out_density);
@@ -395,7 +465,9 @@ int ffpp_run_host(ffpp_handle* h, const void* raw, int32_t B, const int32_t* N_p
 int ffpp_destroy(ffpp_handle* h) {
   if (!h) return FFPP_OK;
   cudaFree(h->d_meta); cudaFree(h->d_surv_keys); cudaFree(h->d_counters); cudaFree(h->d_sorted_box);
-  cudaFree(h->d_sorted_logit); cudaFree(h->d_sorted_idx); cudaFree(h->d_mask);
+  cudaFree(h->d_sorted_logit); cudaFree(h->d_sorted_idx); cudaFree(h->d_mask); cudaFree(h->d_hist32);
+  cudaFree(h->d_sp_box); cudaFree(h->d_sp_rank); cudaFree(h->d_nzc); cudaFree(h->d_bbox32); cudaFree(h->d_slot_base);
+  cudaFree(h->d_W32); cudaFree(h->d_WQ);
   cudaFree(h->d_in); cudaFree(h->d_out_boxes); cudaFree(h->d_out_counts); cudaFree(h->d_out_density);
   if (h->h_meta) cudaFreeHost(h->h_meta);
   if (h->meta_done) cudaEventDestroy(h->meta_done);

@@ -58,11 +58,19 @@ def test_config2_fp16(torch_cuda, ffpp_mod, oracle_mod, gen_mod, seed):
     compare(out, ref, w, check_stage=pp)
 
 
+@pytest.mark.parametrize("nms_mode", [0, 1])
 @pytest.mark.parametrize("c,B", [(3, 4), (4, 3), (5, 8)])
-def test_larger_configs_reduced_batch(torch_cuda, ffpp_mod, oracle_mod, gen_mod, c, B):
+def test_larger_configs_reduced_batch(torch_cuda, ffpp_mod, oracle_mod, gen_mod, c, B, nms_mode):
     w = gen_mod.make_config(c, B=B)
-    pp, out, ref = run_both(torch_cuda, ffpp_mod, oracle_mod, w)
+    pp, out, ref = run_both(torch_cuda, ffpp_mod, oracle_mod, w, nms_mode=nms_mode)
     compare(out, ref, w, check_stage=pp)
+
+
+def test_dense_mode_small_configs(torch_cuda, ffpp_mod, oracle_mod, gen_mod):
+    for c in (1, 2):
+        w = gen_mod.make_config(c)
+        pp, out, ref = run_both(torch_cuda, ffpp_mod, oracle_mod, w, nms_mode=1)
+        compare(out, ref, w, check_stage=pp)
 
 
 def test_determinism_and_reuse_of_a_handle(torch_cuda, ffpp_mod, oracle_mod, gen_mod):
