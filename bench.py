@@ -284,37 +284,54 @@ def run_ours(args):
         key_b = info.key_bits // 8
         cell_b = 4 * cells
         kept_n = int(kept.sum())
-        # algorithmic bytes / ops per launch
-        a1_bytes = total_cand * 5 * elem + int(n_surv.sum()) * key_b
-        a56_bytes = cell_b + 16 * kept_n
+        # algorithmic bytes / ops per launch (DESIGN.md §6 "Kernels and rooflines")
+        row_b = 5 * elem
+        n_sv, n_in = int(n_surv.sum()), int(n_sorted.sum())
+        alg_bytes = {
+            "a1_threshold_compact": total_cand * row_b + n_sv * key_b,           # read every row once, write one key per survivor
+            "a2_sort_topk_decode": n_sv * key_b + n_in * (row_b + 24),            # read keys, gather top-K rows, write box+logit+index
+            "a4_nms_sweep": n_in * 24 + kept_n * 24 + 4 * B,                      # read sorted records, write kept records + counts
+            "a5a6_density": cell_b + 16 * kept_n,                                 # read kept boxes, write every density cell once
+        }
         stages = {}
         names = ffpp.STAGE_NAMES
         for i, nm in enumerate(names):
-            stages[nm] = {"ms": float(stage_ms[i])}
-        s1 = stages["a1_threshold_compact"]; s1["algorithmic_bytes"] = a1_bytes
-        s1["GB/s"] = a1_bytes / (stage_ms[1] * 1e-3) / 1e9; s1["frac_of_hbm_peak"] = s1["GB/s"] / hbm_peak
-        s5 = stages["a5a6_density"]; s5["algorithmic_bytes"] = a56_bytes
-        s5["GB/s"] = a56_bytes / (stage_ms[5] * 1e-3) / 1e9; s5["frac_of_hbm_peak"] = s5["GB/s"] / hbm_peak
+            stages[nm] = {"ms": float(stage_ms[i]), "share_of_step": float(stage_ms[i] / stage_ms.sum())}
+            if nm in alg_bytes:
+                gbs = alg_bytes[nm] / (stage_ms[i] * 1e-3) / 1e9
+                stages[nm].update({"algorithmic_bytes": alg_bytes[nm], "GB/s": gbs, "frac_of_hbm_peak": gbs / hbm_peak})
         s3 = stages["a3_nms_mask"]; s3["iou_pairs"] = pairs
         s3["Gpairs/s"] = pairs / (stage_ms[3] * 1e-3) / 1e9
+        # a3 ALU ceiling of the all-pairs method: 148 SM x 128 fp32 lanes x clock / 15 instr per IoU pair
+        alu_peak_gpairs = 148 * 128 * sm_max_mhz * 1e6 / ffpp.NMS_ALU_OPS_PER_PAIR / 1e9
+        s3["frac_of_allpairs_alu_peak"] = s3["Gpairs/s"] / alu_peak_gpairs
         # dominant kernel = the stage with the largest share of the step
         dom = int(np.argmax(stage_ms[1:])) + 1
-        alu_peak_gpairs = 148 * 128 * sm_max_mhz * 1e6 / ffpp.NMS_ALU_OPS_PER_PAIR / 1e9
         if dom == 3:
-            roofline = {"kernel": "k3_nms_mask", "bound": "alu", "achieved": s3["Gpairs/s"], "peak": alu_peak_gpairs,
+            roofline = {"kernel": ffpp.STAGE_KERNELS[names[dom]], "bound": "alu", "achieved": s3["Gpairs/s"], "peak": alu_peak_gpairs,
                         "unit": "Gpair/s", "frac": s3["Gpairs/s"] / alu_peak_gpairs, "traffic": None,
-                        "peak_source": f"148 SM x 128 fp32 lanes x {sm_max_mhz:.0f} MHz / {ffpp.NMS_ALU_OPS_PER_PAIR} ALU ops per IoU pair "
-                                       "(DESIGN.md §Kernels a3)"}
+                        "peak_source": f"148 SM x 128 fp32 lanes x {sm_max_mhz:.0f} MHz / {ffpp.NMS_ALU_OPS_PER_PAIR} fp32 instr per IoU pair "
+                                       "(SURVEY §8(d) all-pairs ceiling; DESIGN.md §6 a3)",
+                        "note": "pairs = full upper triangle n'(n'-1)/2 per frame that the launch DECIDES; the spatially tiled kernel "
+                                "decides most of them by bounding-box culling without evaluating them, so frac > 1 is possible and "
+                                "means 'faster than the all-pairs method can go', not 'above the hardware'"}
         else:
             sd = stages[names[dom]]
-            ab = sd.get("algorithmic_bytes")
-            roofline = {"kernel": names[dom], "bound": "hbm", "achieved": sd.get("GB/s"), "peak": hbm_peak, "unit": "GB/s",
-                        "frac": (sd.get("GB/s") / hbm_peak) if ab else None, "traffic": None, "peak_source": peak_src}
+            roofline = {"kernel": ffpp.STAGE_KERNELS[names[dom]], "bound": "hbm", "achieved": sd["GB/s"], "peak": hbm_peak, "unit": "GB/s",
+                        "frac": sd["GB/s"] / hbm_peak, "traffic": None, "peak_source": peak_src}
+        roofline["stage"] = names[dom]
+        roofline["avg_launch_ms"] = float(stage_ms[dom])
         roofline["hbm_peak_source"] = peak_src
         tr_path = os.path.join(ROOT, "profiles", f"traffic_config{c}.json")
         if os.path.exists(tr_path):      # dram bytes per launch from the committed ncu --set full capture
             with open(tr_path) as fh:
                 roofline["traffic"] = json.load(fh).get(roofline["kernel"])
+        # whole step against HBM: bytes the path must move (raw in, three outputs out) / device step time
+        step_bytes = total_cand * row_b + 24 * kept_n + 4 * B + cell_b
+        step_gbs = step_bytes / (float(np.median(step_ms)) * 1e-3) / 1e9
+        step_roofline = {"bound": "hbm", "algorithmic_bytes": step_bytes, "achieved": step_gbs, "peak": hbm_peak, "unit": "GB/s",
+                         "frac": step_gbs / hbm_peak, "note": "raw head output read once + kept boxes, counts and density written once, "
+                         "over the median device step time of this rank; every intermediate is overhead against this bound"}
 
         # ---- CPU baseline: the oracle as it stands on this box's host cores, bounded sample ----
         cpu = None
@@ -342,6 +359,7 @@ def run_ours(args):
                     "api": "ffpp_run_host (pinned host buffers, copies + sync inside the timed region)"},
             "gpu_launches": 5 * K,
             "roofline": roofline,
+            "step_roofline": step_roofline,
             "stages": stages,
             "cpu_baseline": cpu,
             "clocks": clocks,

@@ -31,9 +31,14 @@ FFPP_OK, FFPP_EINVAL, FFPP_ECAPACITY, FFPP_ECUDA, FFPP_ENOMEM = 0, -1, -2, -3, -
 NUM_STAGES = 6
 STAGE_NAMES = ["a0_schedule", "a1_threshold_compact", "a2_sort_topk_decode", "a3_nms_mask", "a4_nms_sweep", "a5a6_density"]
 
-# ALU ops per IoU pair that any all-pairs bitmask NMS must issue: the four chained compare-and-AND of the strict
-# overlap test (DESIGN.md §Kernels a3).  bench.py divides the fp32 lane rate by this to get the pairs/s ceiling.
-NMS_ALU_OPS_PER_PAIR = 4
+STAGE_KERNELS = {"a0_schedule": "host scheduler + memset", "a1_threshold_compact": "k1_threshold_compact",
+                 "a2_sort_topk_decode": "k2_sort_topk_decode", "a3_nms_mask": "k3_nms_tiles", "a4_nms_sweep": "k4_resolve_emit",
+                 "a5a6_density": "k5_density"}
+
+# fp32 instructions per IoU pair of the all-pairs bitmask method (4 min/max, 2 sub, 2 clamp, 1 mul, area
+# add/sub, divide-or-multiply + compare = 12-16; 15 taken).  bench.py divides the fp32 lane rate by this to get the
+# pairs/s ceiling of the all-pairs method (DESIGN.md §6 a3).
+NMS_ALU_OPS_PER_PAIR = 15
 
 BOX_DTYPE = np.dtype([("x1", "<f4"), ("y1", "<f4"), ("x2", "<f4"), ("y2", "<f4"), ("score", "<f4"), ("cand_index", "<i4")])
 
