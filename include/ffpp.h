@@ -52,13 +52,12 @@ typedef struct ffpp_params {
   int32_t max_frame_w;     /* capacity: W_f <= max_frame_w                                                          */
   int32_t max_frame_h;     /* capacity: H_f <= max_frame_h                                                          */
   int64_t max_total_cells; /* capacity: sum_f (W_f/cell)(H_f/cell); 0 = max_frames * (max_w/cell)(max_h/cell)       */
-  int64_t nms_workspace_bytes; /* capacity of the NMS suppression-word workspace; 0 = default: tiled mode
-                                  nms_slots_per_block slots per 32-box block, dense mode the worst case for
-                                  max_frames frames of min(top_k, max candidates of a max_w x max_h frame) boxes   */
-  int32_t nms_mode;        /* 0 = spatially tiled suppression words (default); 1 = dense rank-order 64x64 bitmask
-                              + single-warp sweep.  Both compute the same greedy NMS (O5)           */
-  int32_t nms_slots_per_block; /* tiled mode: suppression-word slots (192 B each) reserved per 32-box block;
-                                  0 = 64.  A block that needs more falls back to recomputing its words            */
+  int64_t nms_workspace_bytes; /* capacity of the NMS suppression-edge pool in bytes (4 per edge, shared out to the
+                                  frames in proportion to min(N_f, top_k)); 0 = nms_edges_per_box edges per box       */
+  int32_t nms_edges_per_box; /* 0 = 32.  An edge is one pair (a, b) with IoU > iou_thresh, b before a in the order; the
+                                flock workloads have 4-8 per box.  A frame that needs more than its share reports
+                                out_counts[f] = -1 and leaves its out_boxes / out_density rows undefined              */
+  int32_t reserved_;
 } ffpp_params;
 
 /* One kept detection (24 bytes).  score = sigmoid(logit) in fp32; cand_index = candidate index within its frame. */
@@ -121,8 +120,8 @@ int ffpp_get_info(const ffpp_handle* h, ffpp_info* out /*HOST*/);
 /* Stage timing.  When enabled, ffpp_run records CUDA events on `stream` around each stage of the NEXT runs;
  * ffpp_get_stage_ms (after the caller synchronised the stream) returns the last run's durations in ms:
  *   [0] scheduler upload + counter reset   (a0)      [1] decode/threshold/compaction        (a1)
- *   [2] segmented sort + top-K + decode    (a2)      [3] NMS suppression bitmask            (a3)
- *   [4] NMS sweep + output gather          (a4)      [5] density histogram + convolution    (a5-a6)
+ *   [2] top-K select + decode + spatial bin (a2)     [3] NMS suppression edges              (a3)
+ *   [4] NMS resolve + order + output gather (a4)      [5] density histogram + convolution    (a5-a6)
  * Event recording makes the run non-capturable; leave it off for graph capture. */
 #define FFPP_NUM_STAGES 6
 int ffpp_set_stage_timing(ffpp_handle* h, int32_t enable);
@@ -131,8 +130,9 @@ int ffpp_get_stage_ms(ffpp_handle* h, float* ms_out /*HOST [FFPP_NUM_STAGES]*/);
 /* Test-only readback of per-stage intermediates of the LAST run (synchronises the device).
  *   what = 0: survivor count per frame after thresholding       dst HOST int32 [B]
  *   what = 1: sorted count per frame  min(n, top_k)             dst HOST int32 [B]
- *   what = 2: sorted candidate indices                          dst HOST int32 [B][top_k] (rows past the count: -1)
- *   what = 3: sorted decoded boxes                              dst HOST float [B][top_k][4]
+ *   what = 2: candidate indices of the top-K set in the order   dst HOST int32 [B][top_k] (rows past the count: -1)
+ *             of O4 (the device holds the set with its keys in spatial order; the readback sorts by key on the host)
+ *   what = 3: decoded boxes of the top-K set, same order        dst HOST float [B][top_k][4]
  * Not part of the contract of the path; used to localise a parity failure. */
 int ffpp_debug_read(ffpp_handle* h, int32_t what, void* dst /*HOST*/, int64_t dst_bytes);
 

@@ -21,7 +21,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 _LIB = os.path.join(_HERE, "libffpp.so")
-_SOURCES = ["ffpp.cu", "ffpp_kernels.cuh", "ffpp_nms_dense.cuh", "ffpp_common.cuh"]
+_SOURCES = ["ffpp.cu", "ffpp_kernels.cuh", "ffpp_common.cuh"]
 _INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
@@ -32,7 +32,7 @@ NUM_STAGES = 6
 STAGE_NAMES = ["a0_schedule", "a1_threshold_compact", "a2_sort_topk_decode", "a3_nms_mask", "a4_nms_sweep", "a5a6_density"]
 
 STAGE_KERNELS = {"a0_schedule": "host scheduler + memset", "a1_threshold_compact": "k1_threshold_compact",
-                 "a2_sort_topk_decode": "k2_sort_topk_decode", "a3_nms_mask": "k3_nms_tiles", "a4_nms_sweep": "k4_resolve_emit",
+                 "a2_sort_topk_decode": "k2_select_bin", "a3_nms_mask": "k3_nms_edges", "a4_nms_sweep": "k4_resolve_emit",
                  "a5a6_density": "k5_density"}
 
 # fp32 instructions per IoU pair of the all-pairs bitmask method (4 min/max, 2 sub, 2 clamp, 1 mul, area
@@ -54,7 +54,7 @@ class FFPPParams(ctypes.Structure):
         ("max_frames", ctypes.c_int32), ("max_total_candidates", ctypes.c_int64),
         ("max_frame_w", ctypes.c_int32), ("max_frame_h", ctypes.c_int32),
         ("max_total_cells", ctypes.c_int64), ("nms_workspace_bytes", ctypes.c_int64),
-        ("nms_mode", ctypes.c_int32), ("nms_slots_per_block", ctypes.c_int32),
+        ("nms_edges_per_box", ctypes.c_int32), ("reserved_", ctypes.c_int32),
     ]
 
 
@@ -114,8 +114,7 @@ def load_library() -> ctypes.CDLL:
 
 
 def make_params(params: dict, *, max_frames: int, max_total_candidates: int, max_frame_w: int, max_frame_h: int,
-                max_total_cells: int = 0, nms_workspace_bytes: int = 0, nms_mode: int = 0,
-                nms_slots_per_block: int = 0) -> FFPPParams:
+                max_total_cells: int = 0, nms_workspace_bytes: int = 0, nms_edges_per_box: int = 0) -> FFPPParams:
     p = FFPPParams()
     p.dtype = 1 if params["dtype"] == "fp16" else 0
     p.conf_thresh = params["conf_thresh"]
@@ -133,8 +132,7 @@ def make_params(params: dict, *, max_frames: int, max_total_candidates: int, max
     p.max_frame_w, p.max_frame_h = max_frame_w, max_frame_h
     p.max_total_cells = max_total_cells
     p.nms_workspace_bytes = nms_workspace_bytes
-    p.nms_mode = nms_mode
-    p.nms_slots_per_block = nms_slots_per_block
+    p.nms_edges_per_box = nms_edges_per_box
     return p
 
 
@@ -158,7 +156,7 @@ class FFPP:
     """One libffpp handle (ffpp_create / ffpp_destroy) on the current CUDA device."""
 
     def __init__(self, params: dict, *, max_frames: int, max_total_candidates: int, max_frame_w: int, max_frame_h: int,
-                 max_total_cells: int = 0, nms_workspace_bytes: int = 0, nms_mode: int = 0, nms_slots_per_block: int = 0):
+                 max_total_cells: int = 0, nms_workspace_bytes: int = 0, nms_edges_per_box: int = 0):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2512_07009_b200 needs a CUDA sm_100 device; there is no CPU fallback")
@@ -172,8 +170,7 @@ class FFPP:
         self._torch_dtype = torch.float16 if params["dtype"] == "fp16" else torch.float32
         self._p = make_params(params, max_frames=max_frames, max_total_candidates=max_total_candidates,
                               max_frame_w=max_frame_w, max_frame_h=max_frame_h, max_total_cells=max_total_cells,
-                              nms_workspace_bytes=nms_workspace_bytes, nms_mode=nms_mode,
-                              nms_slots_per_block=nms_slots_per_block)
+                              nms_workspace_bytes=nms_workspace_bytes, nms_edges_per_box=nms_edges_per_box)
         self._h = ctypes.c_void_p()
         rc = self._lib.ffpp_create(ctypes.byref(self._p), ctypes.byref(self._h))
         if rc != FFPP_OK:

@@ -9,7 +9,6 @@
 #include <vector>
 
 #include "ffpp_kernels.cuh"
-#include "ffpp_nms_dense.cuh"
 
 using namespace ffpp;
 
@@ -18,7 +17,7 @@ namespace {
 thread_local std::string g_create_error;
 
 struct DeviceMeta {           // one pinned block + one device block, uploaded with a single copy
-  size_t frames_off, cand_off_off, unit_prefix_off, bytes;
+  size_t frames_off, cand_off_off, bytes;
 };
 
 DeviceMeta meta_layout(int max_frames) {
@@ -27,7 +26,6 @@ DeviceMeta meta_layout(int max_frames) {
   m.frames_off = o; o += sizeof(FrameDesc) * (size_t)max_frames;
   o = (o + 15) & ~(size_t)15;
   m.cand_off_off = o; o += sizeof(int64_t) * ((size_t)max_frames + 1);
-  m.unit_prefix_off = o; o += sizeof(int32_t) * ((size_t)max_frames + 1);
   m.bytes = (o + 15) & ~(size_t)15;
   return m;
 }
@@ -38,35 +36,28 @@ struct ffpp_handle {
   ffpp_params p;
   Consts cst;
   bool half = false;
-  bool dense = false;                 // nms_mode == 1
   int key_bytes = 8;
-  int key_slots = 0;                  // a2: keys staged in shared memory
-  int nb32cap = 0;                    // ceil(top_k / 32): stride of the per-block arrays
+  int kpad = 0;                       // top_k rounded up to 32: per-frame stride of the spatial arrays
+  int nb32cap = 0, nb8cap = 0;        // kpad / 32, kpad / 8
   int sm_count = 148;
   int max_frame_cand = 0;
   int64_t max_total_cells = 0;
-  int64_t mask_words_cap = 0;         // dense mode: uint64 words
-  int64_t slot_cap_total = 0;         // tiled mode: suppression-word slots (32 words each)
+  int64_t edge_cap_total = 0;         // suppression-edge pool, entries
+  int64_t edges_per_box = 32;
   std::string err;
 
   // device workspace
   uint8_t* d_meta = nullptr;
   void* d_surv_keys = nullptr;
-  int* d_counters = nullptr;          // 4 x max_frames: survivor counts | sorted counts | slot counters | frame_err
-  float4* d_sorted_box = nullptr;
-  float* d_sorted_logit = nullptr;
-  int* d_sorted_idx = nullptr;
-  uint32_t* d_hist32 = nullptr;       // a5: uint16 count per density cell, two per word
-  // tiled NMS
-  float4* d_sp_box = nullptr;
-  uint16_t* d_sp_rank = nullptr;
+  int* d_counters = nullptr;          // 4 x max_frames: survivor counts | top-K counts | edge counters | frame_err
+  float4* d_sel_box = nullptr;        // a2 scratch: decoded boxes in selection order
+  float4* d_sp_box = nullptr;         // spatial (Hilbert) order, stride kpad per frame
+  float4* d_sp_sbox = nullptr;        // culling boxes
+  void* d_sp_key = nullptr;
+  float4* d_bbox8 = nullptr;
   float4* d_bbox32 = nullptr;
-  int* d_slot_base = nullptr;
-  uint16_t* d_nzc = nullptr;
-  uint32_t* d_W32 = nullptr;
-  uint16_t* d_WQ = nullptr;
-  // dense NMS
-  unsigned long long* d_mask = nullptr;
+  uint32_t* d_edges = nullptr;
+  uint32_t* d_hist32 = nullptr;       // a5: uint16 count per density cell, two per word
   int64_t workspace_bytes = 0;
   // pinned staging for the descriptor table
   uint8_t* h_meta = nullptr;
@@ -75,7 +66,7 @@ struct ffpp_handle {
   // geometry of the last batch (skip rebuild + upload when unchanged)
   int last_B = -1;
   std::vector<int32_t> last_N, last_dims;
-  int total_units = 0, max_tiles = 0, max_nmax = 0;
+  int max_tiles = 0, max_nmax = 0;
   int64_t total_cand = 0, total_cells = 0;
   // host-buffer path staging (allocated on first ffpp_run_host)
   void* d_in = nullptr;
@@ -89,7 +80,7 @@ struct ffpp_handle {
 
   int* surv_cnt() const { return d_counters; }
   int* n_sorted() const { return d_counters + p.max_frames; }
-  int* slot_ctr() const { return d_counters + 2 * (size_t)p.max_frames; }
+  int* edge_ctr() const { return d_counters + 2 * (size_t)p.max_frames; }
   int* frame_err() const { return d_counters + 3 * (size_t)p.max_frames; }
 };
 
@@ -119,7 +110,7 @@ int64_t frame_candidates(const ffpp_params& p, int W, int H) {
   return n;
 }
 
-// a0: validate the batch, (re)build the descriptor table + work-list prefixes, upload if the geometry changed.
+// a0: validate the batch, (re)build the descriptor table, upload if the geometry changed.
 int schedule(ffpp_handle* h, int B, const int32_t* N, const int32_t* dims, cudaStream_t stream) {
   const ffpp_params& p = h->p;
   if (B == h->last_B && std::memcmp(N, h->last_N.data(), sizeof(int32_t) * B) == 0 &&
@@ -130,10 +121,9 @@ int schedule(ffpp_handle* h, int B, const int32_t* N, const int32_t* dims, cudaS
   h->last_B = -1;
   FrameDesc* fr = reinterpret_cast<FrameDesc*>(h->h_meta + h->ml.frames_off);
   int64_t* coff = reinterpret_cast<int64_t*>(h->h_meta + h->ml.cand_off_off);
-  int32_t* uoff = reinterpret_cast<int32_t*>(h->h_meta + h->ml.unit_prefix_off);
   const int smax = p.strides[p.num_levels - 1];
   const int R = h->cst.radius;
-  int64_t cand = 0, cells = 0, mwords = 0, units = 0, slots = 0;
+  int64_t cand = 0, cells = 0, edges = 0;
   int max_tiles = 0, max_nmax = 0;
   for (int f = 0; f < B; ++f) {
     const int W = dims[2 * f], H = dims[2 * f + 1];
@@ -160,22 +150,11 @@ int schedule(ffpp_handle* h, int B, const int32_t* N, const int32_t* dims, cudaS
     d.gw = W / p.cell_px; d.gh = H / p.cell_px;
     if (d.gw < R || d.gh < R) return fail(h, FFPP_EINVAL, "density grid smaller than the Gaussian radius");
     int hs = 0;
-    while ((256 << hs) < std::max(W, H)) ++hs;
+    while ((128 << hs) < std::max(W, H)) ++hs;
     d.hshift = hs;
-    if (h->dense) {
-      d.nbmax = (d.nmax + kNmsTile - 1) / kNmsTile;
-      d.mask_off = mwords;
-      mwords += mask_words(d.nbmax);
-      uoff[f] = (int32_t)units;
-      units += k3d_units(d.nbmax);
-      if (units > 0x7fffffff) return fail(h, FFPP_ECAPACITY, "work list too large");
-    } else {
-      const int64_t nb = (d.nmax + kBlk - 1) / kBlk;
-      d.slot_off = slots;
-      d.slot_cap = (int32_t)std::min<int64_t>(nb * nb, nb * h->p.nms_slots_per_block);
-      slots += d.slot_cap;
-      uoff[f] = 0;
-    }
+    d.edge_off = edges;
+    d.edge_cap = (int32_t)std::min<int64_t>(h->edges_per_box * d.nmax, 0x7fffffff);
+    edges += d.edge_cap;
     fr[f] = d;
     coff[f] = cand;
     cand += n; cells += (int64_t)d.gw * d.gh;
@@ -183,17 +162,16 @@ int schedule(ffpp_handle* h, int B, const int32_t* N, const int32_t* dims, cudaS
     max_tiles = std::max(max_tiles, tiles);
     max_nmax = std::max(max_nmax, (int)d.nmax);
   }
-  coff[B] = cand; uoff[B] = (int32_t)units;
+  coff[B] = cand;
   if (cand > p.max_total_candidates) return fail(h, FFPP_ECAPACITY, "sum N_f exceeds max_total_candidates");
   if (cells > h->max_total_cells) return fail(h, FFPP_ECAPACITY, "density cells exceed max_total_cells");
-  if (mwords > h->mask_words_cap) return fail(h, FFPP_ECAPACITY, "suppression mask exceeds nms_workspace_bytes");
-  if (slots > h->slot_cap_total) return fail(h, FFPP_ECAPACITY, "suppression-word pool exceeds nms_workspace_bytes");
+  if (edges > h->edge_cap_total) return fail(h, FFPP_ECAPACITY, "suppression-edge pool exceeds nms_workspace_bytes");
   FFPP_CUDA(h, cudaMemcpyAsync(h->d_meta, h->h_meta, h->ml.bytes, cudaMemcpyHostToDevice, stream));
   FFPP_CUDA(h, cudaEventRecord(h->meta_done, stream));
   h->last_B = B;
   h->last_N.assign(N, N + B);
   h->last_dims.assign(dims, dims + 2 * B);
-  h->total_units = (int)units; h->max_tiles = max_tiles; h->max_nmax = max_nmax;
+  h->max_tiles = max_tiles; h->max_nmax = max_nmax;
   h->total_cand = cand; h->total_cells = cells;
   return FFPP_OK;
 }
@@ -203,7 +181,6 @@ int launch_all(ffpp_handle* h, const void* raw, int B, cudaStream_t st, ffpp_box
                float* out_density) {
   const FrameDesc* frames = reinterpret_cast<const FrameDesc*>(h->d_meta + h->ml.frames_off);
   const int64_t* coff = reinterpret_cast<const int64_t*>(h->d_meta + h->ml.cand_off_off);
-  const int32_t* uoff = reinterpret_cast<const int32_t*>(h->d_meta + h->ml.unit_prefix_off);
   const Consts& c = h->cst;
   const bool tm = h->timing;
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[1], st));
@@ -220,30 +197,24 @@ int launch_all(ffpp_handle* h, const void* raw, int B, cudaStream_t st, ffpp_box
   }
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[2], st));
   // a2 (+ clears the a5 histogram)
-  k2_sort_topk_decode<kHalf, KeyT><<<B, K2_THREADS, k2_smem_bytes((size_t)h->key_slots, sizeof(KeyT)), st>>>(
-      static_cast<const uint8_t*>(raw), frames, static_cast<const KeyT*>(h->d_surv_keys), h->surv_cnt(), c, h->key_slots,
-      h->nb32cap, h->d_sorted_box, h->d_sorted_logit, h->d_sorted_idx, h->n_sorted(), h->d_sp_box, h->d_sp_rank,
-      h->d_bbox32, h->d_hist32, h->dense ? 0 : 1);
+  k2_select_bin<kHalf, KeyT><<<B, K2_THREADS, k2_smem_bytes((size_t)c.top_k, sizeof(KeyT)), st>>>(
+      static_cast<const uint8_t*>(raw), frames, static_cast<const KeyT*>(h->d_surv_keys), h->surv_cnt(), c, h->nb8cap,
+      h->nb32cap, h->d_sel_box, h->d_sp_box, h->d_sp_sbox, static_cast<KeyT*>(h->d_sp_key), h->d_bbox8, h->d_bbox32,
+      h->n_sorted(), h->d_hist32);
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[3], st));
-  if (h->dense) {
-    // a3 / a4, dense rank-order bitmask
-    if (h->total_units > 0)
-      k3d_nms_mask<<<h->total_units, K3D_THREADS, 0, st>>>(frames, uoff, B, h->d_sorted_box, h->n_sorted(), c, h->d_mask);
-    if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[4], st));
-    const size_t smem = sizeof(unsigned long long) * (size_t)((h->p.top_k + kNmsTile - 1) / kNmsTile);
-    k4d_nms_sweep<<<B, K4D_THREADS, smem, st>>>(frames, h->d_sorted_box, h->d_sorted_logit, h->d_sorted_idx, h->n_sorted(),
-                                                c, h->d_mask, out_boxes, out_counts, h->d_hist32);
-  } else {
-    // a3 / a4, spatially tiled
+  // a3
+  {
     const dim3 g3((unsigned)((h->max_nmax + K3_THREADS - 1) / K3_THREADS), (unsigned)B);
     if (g3.x > 0)
-      k3_nms_tiles<<<g3, K3_THREADS, 0, st>>>(frames, h->n_sorted(), h->d_sp_box, h->d_sp_rank, h->d_bbox32, c, h->nb32cap,
-                                              h->slot_ctr(), h->d_slot_base, h->d_nzc, h->d_W32, h->d_WQ, h->frame_err());
-    if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[4], st));
-    k4_resolve_emit<<<B, K4_THREADS, 0, st>>>(frames, h->n_sorted(), h->d_sorted_box, h->d_sorted_logit, h->d_sorted_idx,
-                                              h->d_sp_rank, h->d_nzc, h->d_slot_base, h->d_W32, h->d_WQ, h->frame_err(), c,
-                                              h->nb32cap, out_boxes, out_counts, h->d_hist32);
+      k3_nms_edges<KeyT><<<g3, K3_THREADS, 0, st>>>(frames, h->n_sorted(), h->d_sp_box, h->d_sp_sbox,
+                                                    static_cast<const KeyT*>(h->d_sp_key), h->d_bbox8, h->d_bbox32, c,
+                                                    h->nb8cap, h->nb32cap, h->edge_ctr(), h->d_edges, h->frame_err());
   }
+  if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[4], st));
+  // a4 (+ a5 histogram)
+  k4_resolve_emit<KeyT><<<B, K4_THREADS, k4_smem_bytes((size_t)c.top_k, (size_t)c.kpad, sizeof(KeyT)), st>>>(
+      frames, h->n_sorted(), h->d_sp_box, static_cast<const KeyT*>(h->d_sp_key), h->edge_ctr(), h->d_edges, h->frame_err(), c,
+      out_boxes, out_counts, h->d_hist32);
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[5], st));
   // a6
   {
@@ -263,8 +234,10 @@ template <bool kHalf, typename KeyT>
 int set_kernel_attrs(ffpp_handle* h) {
   const size_t s1 = K1_STAGES * K1_CHUNK_BYTES;
   FFPP_CUDA(h, cudaFuncSetAttribute(k1_threshold_compact<kHalf, KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s1));
-  const size_t s2 = k2_smem_bytes((size_t)h->key_slots, sizeof(KeyT));
-  FFPP_CUDA(h, cudaFuncSetAttribute(k2_sort_topk_decode<kHalf, KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s2));
+  const size_t s2 = k2_smem_bytes((size_t)h->p.top_k, sizeof(KeyT));
+  FFPP_CUDA(h, cudaFuncSetAttribute(k2_select_bin<kHalf, KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s2));
+  const size_t s4 = k4_smem_bytes((size_t)h->p.top_k, (size_t)h->kpad, sizeof(KeyT));
+  FFPP_CUDA(h, cudaFuncSetAttribute(k4_resolve_emit<KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s4));
   return FFPP_OK;
 }
 
@@ -290,27 +263,26 @@ int ffpp_create(const ffpp_params* p, ffpp_handle** out) {
   const int R = (int)std::floor((double)p->truncate_sigmas * (double)p->sigma_cells);
   if (R < 1 || R > kMaxRadius) return fail(nullptr, FFPP_EINVAL, "Gaussian radius floor(truncate*sigma) must be 1..32");
 
-  if (p->nms_mode != 0 && p->nms_mode != 1) return fail(nullptr, FFPP_EINVAL, "nms_mode must be 0 (tiled) or 1 (dense)");
-  if (p->nms_slots_per_block < 0) return fail(nullptr, FFPP_EINVAL, "nms_slots_per_block must be >= 0");
+  if (p->nms_edges_per_box < 0 || p->nms_workspace_bytes < 0) return fail(nullptr, FFPP_EINVAL, "nms_edges_per_box / nms_workspace_bytes must be >= 0");
   ffpp_handle* h = new (std::nothrow) ffpp_handle();
   if (!h) return fail(nullptr, FFPP_ENOMEM, "host allocation failed");
   h->p = *p;
   h->half = p->dtype == 1;
-  h->dense = p->nms_mode == 1;
   const int64_t nmaxframe = frame_candidates(*p, p->max_frame_w, p->max_frame_h);
   h->max_frame_cand = (int)std::min<int64_t>(nmaxframe, 1 << 20);
   h->key_bytes = (h->half && nmaxframe <= 65536) ? 4 : 8;
+  h->kpad = (p->top_k + kBlk - 1) / kBlk * kBlk;
+  h->nb32cap = h->kpad / kBlk;
+  h->nb8cap = h->kpad / kSub;
   {
-    // a2 shared-memory budget: everything the 227 KB opt-in limit leaves after the histograms holds keys
-    const size_t fixed = k2_smem_bytes(0, h->key_bytes) + 1024;      // + static shared of the kernel
-    const int64_t fit = (int64_t)((232448 - fixed) / h->key_bytes);
-    if (2 * (int64_t)p->top_k > fit || p->top_k > 24576) {
+    // shared-memory budgets of a2 (selected keys + bin bookkeeping) and a4 (two sort buffers) under the 227 KB opt-in limit
+    const size_t lim = 232448;                                        // minus each kernel's static shared memory
+    if (p->top_k > kMaxTopK || k2_smem_bytes((size_t)p->top_k, h->key_bytes) > lim - 512 ||
+        k4_smem_bytes((size_t)p->top_k, (size_t)h->kpad, h->key_bytes) > lim - 6656) {
       delete h;
-      return fail(nullptr, FFPP_EINVAL, "top_k exceeds the shared-memory sort capacity (24576 with 32-bit keys, 12288 with 64-bit keys)");
+      return fail(nullptr, FFPP_EINVAL, "top_k exceeds the shared-memory capacity (24576 with 32-bit keys, 12288 with 64-bit keys)");
     }
-    h->key_slots = (int)std::min<int64_t>(fit, std::max<int64_t>(2 * (int64_t)p->top_k, h->max_frame_cand));
   }
-  h->nb32cap = (p->top_k + kBlk - 1) / kBlk;
 
   // constants
   Consts& c = h->cst;
@@ -322,7 +294,9 @@ int ffpp_create(const ffpp_params* p, ffpp_handle** out) {
   c.iou_fast = (p->iou_thresh >= 1e-6f && p->iou_thresh <= 1e6f) ? 1 : 0;
   c.iou_thr_hi = std::nextafterf((float)((double)p->iou_thresh * (1.0 + std::ldexp(1.0, -20))), INFINITY);
   c.iou_thr_lo = std::nextafterf((float)((double)p->iou_thresh * (1.0 - std::ldexp(1.0, -20))), -INFINITY);
+  c.shrink = (p->iou_thresh >= 0.05f) ? 0.49f * std::min(p->iou_thresh, 1.0f) : 0.0f;
   c.top_k = p->top_k;
+  c.kpad = h->kpad;
   c.num_levels = p->num_levels;
   for (int l = 0; l < p->num_levels; ++l) c.stride_log2[l] = ilog2(p->strides[l]);
   c.cell_px = p->cell_px;
@@ -346,19 +320,11 @@ int ffpp_create(const ffpp_params* p, ffpp_handle** out) {
   const int64_t cells_frame = (int64_t)(p->max_frame_w / p->cell_px) * (p->max_frame_h / p->cell_px);
   h->max_total_cells = p->max_total_cells > 0 ? p->max_total_cells : cells_frame * p->max_frames;
   const int64_t nmax_cap = std::min<int64_t>(p->top_k, nmaxframe);
-  if (h->dense) {
-    const int nbcap = (int)((nmax_cap + kNmsTile - 1) / kNmsTile);
-    h->mask_words_cap = p->nms_workspace_bytes > 0 ? p->nms_workspace_bytes / 8 : mask_words(nbcap) * p->max_frames;
-  } else {
-    const int64_t nb = (nmax_cap + kBlk - 1) / kBlk;
-    const int64_t slot_bytes = kBlk * (sizeof(uint32_t) + sizeof(uint16_t));
-    int64_t spb = p->nms_slots_per_block > 0 ? p->nms_slots_per_block : 64;
-    if (p->nms_workspace_bytes > 0) spb = std::max<int64_t>(1, p->nms_workspace_bytes / slot_bytes / (nb * p->max_frames));
-    spb = std::min<int64_t>(spb, nb);
-    h->p.nms_slots_per_block = (int32_t)spb;
-    h->slot_cap_total = spb * nb * p->max_frames;
-    if (h->slot_cap_total > 0x7fffffff) return bail(FFPP_EINVAL, "suppression-word pool has more than 2^31 slots");
-  }
+  h->edges_per_box = p->nms_edges_per_box > 0 ? p->nms_edges_per_box : 32;
+  if (p->nms_workspace_bytes > 0)
+    h->edges_per_box = std::max<int64_t>(1, p->nms_workspace_bytes / 4 / (nmax_cap * p->max_frames));
+  h->p.nms_edges_per_box = (int32_t)std::min<int64_t>(h->edges_per_box, 0x7fffffff);
+  h->edge_cap_total = h->edges_per_box * nmax_cap * p->max_frames;
 
   h->ml = meta_layout(p->max_frames);
   auto dalloc = [&](void** ptr, size_t bytes) {
@@ -367,23 +333,18 @@ int ffpp_create(const ffpp_params* p, ffpp_handle** out) {
     if (ee == cudaSuccess) h->workspace_bytes += (int64_t)bytes;
     return ee;
   };
-  const size_t K = (size_t)p->top_k, F = (size_t)p->max_frames;
-  const size_t pool = (size_t)h->slot_cap_total * kBlk;
+  const size_t KP = (size_t)h->kpad, F = (size_t)p->max_frames;
   if ((e = dalloc((void**)&h->d_meta, h->ml.bytes)) != cudaSuccess ||
       (e = dalloc(&h->d_surv_keys, (size_t)p->max_total_candidates * h->key_bytes)) != cudaSuccess ||
       (e = dalloc((void**)&h->d_counters, 4 * F * sizeof(int))) != cudaSuccess ||
-      (e = dalloc((void**)&h->d_sorted_box, F * K * sizeof(float4))) != cudaSuccess ||
-      (e = dalloc((void**)&h->d_sorted_logit, F * K * sizeof(float))) != cudaSuccess ||
-      (e = dalloc((void**)&h->d_sorted_idx, F * K * sizeof(int))) != cudaSuccess ||
-      (e = dalloc((void**)&h->d_hist32, ((size_t)h->max_total_cells / 2 + 2) * sizeof(uint32_t))) != cudaSuccess ||
-      (e = dalloc((void**)&h->d_mask, (size_t)h->mask_words_cap * 8)) != cudaSuccess ||
-      (!h->dense && ((e = dalloc((void**)&h->d_sp_box, F * K * sizeof(float4))) != cudaSuccess ||
-                     (e = dalloc((void**)&h->d_sp_rank, F * K * sizeof(uint16_t))) != cudaSuccess ||
-                     (e = dalloc((void**)&h->d_nzc, F * K * sizeof(uint16_t))) != cudaSuccess ||
-                     (e = dalloc((void**)&h->d_bbox32, F * (size_t)h->nb32cap * sizeof(float4))) != cudaSuccess ||
-                     (e = dalloc((void**)&h->d_slot_base, F * (size_t)h->nb32cap * sizeof(int))) != cudaSuccess ||
-                     (e = dalloc((void**)&h->d_W32, pool * sizeof(uint32_t))) != cudaSuccess ||
-                     (e = dalloc((void**)&h->d_WQ, pool * sizeof(uint16_t))) != cudaSuccess))) {
+      (e = dalloc((void**)&h->d_sel_box, F * KP * sizeof(float4))) != cudaSuccess ||
+      (e = dalloc((void**)&h->d_sp_box, F * KP * sizeof(float4))) != cudaSuccess ||
+      (e = dalloc((void**)&h->d_sp_sbox, F * KP * sizeof(float4))) != cudaSuccess ||
+      (e = dalloc(&h->d_sp_key, F * KP * (size_t)h->key_bytes)) != cudaSuccess ||
+      (e = dalloc((void**)&h->d_bbox8, F * (size_t)h->nb8cap * sizeof(float4))) != cudaSuccess ||
+      (e = dalloc((void**)&h->d_bbox32, F * (size_t)h->nb32cap * sizeof(float4))) != cudaSuccess ||
+      (e = dalloc((void**)&h->d_edges, (size_t)h->edge_cap_total * sizeof(uint32_t))) != cudaSuccess ||
+      (e = dalloc((void**)&h->d_hist32, ((size_t)h->max_total_cells / 2 + 2) * sizeof(uint32_t))) != cudaSuccess) {
     cudaGetLastError();
     return bail(e == cudaErrorMemoryAllocation ? FFPP_ENOMEM : FFPP_ECUDA, std::string("workspace cudaMalloc: ") + cudaGetErrorString(e));
   }
@@ -464,10 +425,9 @@ int ffpp_run_host(ffpp_handle* h, const void* raw, int32_t B, const int32_t* N_p
 
 int ffpp_destroy(ffpp_handle* h) {
   if (!h) return FFPP_OK;
-  cudaFree(h->d_meta); cudaFree(h->d_surv_keys); cudaFree(h->d_counters); cudaFree(h->d_sorted_box);
-  cudaFree(h->d_sorted_logit); cudaFree(h->d_sorted_idx); cudaFree(h->d_mask); cudaFree(h->d_hist32);
-  cudaFree(h->d_sp_box); cudaFree(h->d_sp_rank); cudaFree(h->d_nzc); cudaFree(h->d_bbox32); cudaFree(h->d_slot_base);
-  cudaFree(h->d_W32); cudaFree(h->d_WQ);
+  cudaFree(h->d_meta); cudaFree(h->d_surv_keys); cudaFree(h->d_counters); cudaFree(h->d_sel_box); cudaFree(h->d_sp_box);
+  cudaFree(h->d_sp_sbox); cudaFree(h->d_sp_key); cudaFree(h->d_bbox8); cudaFree(h->d_bbox32); cudaFree(h->d_edges);
+  cudaFree(h->d_hist32);
   cudaFree(h->d_in); cudaFree(h->d_out_boxes); cudaFree(h->d_out_counts); cudaFree(h->d_out_density);
   if (h->h_meta) cudaFreeHost(h->h_meta);
   if (h->meta_done) cudaEventDestroy(h->meta_done);
@@ -516,26 +476,40 @@ int ffpp_debug_read(ffpp_handle* h, int32_t what, void* dst, int64_t dst_bytes) 
     FFPP_CUDA(h, cudaMemcpy(dst, what == 0 ? h->surv_cnt() : h->n_sorted(), sizeof(int) * B, cudaMemcpyDeviceToHost));
     return FFPP_OK;
   }
+  if (what != 2 && what != 3) return fail(h, FFPP_EINVAL, "unknown debug selector");
+  if (dst_bytes < (int64_t)((what == 2 ? sizeof(int) : 4 * sizeof(float)) * B * K)) return fail(h, FFPP_EINVAL, "dst too small");
+  // the device holds the top-K set in spatial order with its keys; the order of O4 is ascending key
   std::vector<int> ns((size_t)B);
   FFPP_CUDA(h, cudaMemcpy(ns.data(), h->n_sorted(), sizeof(int) * B, cudaMemcpyDeviceToHost));
-  if (what == 2) {
-    if (dst_bytes < (int64_t)(sizeof(int) * B * K)) return fail(h, FFPP_EINVAL, "dst too small");
-    int* d = static_cast<int*>(dst);
-    FFPP_CUDA(h, cudaMemcpy(d, h->d_sorted_idx, sizeof(int) * B * K, cudaMemcpyDeviceToHost));
-    for (int f = 0; f < B; ++f)
-      for (size_t k = (size_t)ns[(size_t)f]; k < K; ++k) d[(size_t)f * K + k] = -1;
-    return FFPP_OK;
+  const size_t KP = (size_t)h->kpad;
+  std::vector<uint64_t> keys(KP);
+  std::vector<float4> boxes(KP);
+  std::vector<uint32_t> k32(KP);
+  std::vector<int> order(KP);
+  for (int f = 0; f < B; ++f) {
+    const int n = ns[(size_t)f];
+    if (h->key_bytes == 4) {
+      FFPP_CUDA(h, cudaMemcpy(k32.data(), static_cast<const uint32_t*>(h->d_sp_key) + (size_t)f * KP, sizeof(uint32_t) * n, cudaMemcpyDeviceToHost));
+      for (int i = 0; i < n; ++i) keys[(size_t)i] = k32[(size_t)i];
+    } else {
+      FFPP_CUDA(h, cudaMemcpy(keys.data(), static_cast<const uint64_t*>(h->d_sp_key) + (size_t)f * KP, sizeof(uint64_t) * n, cudaMemcpyDeviceToHost));
+    }
+    for (int i = 0; i < n; ++i) order[(size_t)i] = i;
+    std::sort(order.begin(), order.begin() + n, [&](int x, int y) { return keys[(size_t)x] < keys[(size_t)y]; });
+    if (what == 2) {
+      int* d = static_cast<int*>(dst) + (size_t)f * K;
+      const uint64_t imask = h->key_bytes == 4 ? 0xFFFFull : 0xFFFFFFFFull;
+      for (int k = 0; k < n; ++k) d[k] = (int)(keys[(size_t)order[(size_t)k]] & imask);
+      for (size_t k = (size_t)n; k < K; ++k) d[k] = -1;
+    } else {
+      FFPP_CUDA(h, cudaMemcpy(boxes.data(), h->d_sp_box + (size_t)f * KP, sizeof(float4) * n, cudaMemcpyDeviceToHost));
+      float* d = static_cast<float*>(dst) + (size_t)f * K * 4;
+      for (int k = 0; k < n; ++k) std::memcpy(d + 4 * (size_t)k, &boxes[(size_t)order[(size_t)k]], sizeof(float4));
+      for (size_t k = (size_t)n * 4; k < K * 4; ++k) d[k] = 0.0f;
+    }
   }
-  if (what == 3) {
-    if (dst_bytes < (int64_t)(sizeof(float) * 4 * B * K)) return fail(h, FFPP_EINVAL, "dst too small");
-    float* d = static_cast<float*>(dst);
-    FFPP_CUDA(h, cudaMemcpy(d, h->d_sorted_box, sizeof(float) * 4 * B * K, cudaMemcpyDeviceToHost));
-    for (int f = 0; f < B; ++f)
-      for (size_t k = (size_t)ns[(size_t)f]; k < K; ++k)
-        for (int e = 0; e < 4; ++e) d[((size_t)f * K + k) * 4 + e] = 0.0f;
-    return FFPP_OK;
-  }
-  return fail(h, FFPP_EINVAL, "unknown debug selector");
+  return FFPP_OK;
+
 }
 
 }  // extern "C"

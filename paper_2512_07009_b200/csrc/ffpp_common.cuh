@@ -10,25 +10,23 @@ namespace ffpp {
 
 constexpr int kMaxLevels = 4;
 constexpr int kMaxRadius = 32;
-constexpr int kNmsTile = 64;        // dense mode: IoU tile edge = bits per suppression word
-constexpr int kBlk = 32;            // tiled mode: boxes per spatial block = bits per suppression word = one warp
+constexpr int kBlk = 32;            // boxes per spatial block = one warp of rows
+constexpr int kSub = 8;             // boxes per spatial sub-block (culling granularity of a3)
+constexpr int kMaxTopK = 24576;
 
 // ---- a0: frame descriptor table (device copy built by the host scheduler, one per frame) ----
 struct FrameDesc {
   int64_t cand_off;                 // first row of the frame in the flat candidate stream
-  int64_t mask_off;                 // dense mode: first uint64 word of the frame's suppression mask
   int64_t dens_off;                 // first float of the frame's density grid (= first uint16 of its histogram)
-  int64_t slot_off;                 // tiled mode: first suppression-word slot of the frame's pool
-  int32_t slot_cap;                 // tiled mode: slots in the frame's pool
+  int64_t edge_off;                 // first entry of the frame's suppression-edge pool
+  int32_t edge_cap;                 // entries in the frame's pool
   int32_t N;                        // candidates
   int32_t W, H;                     // pixels
   int32_t nmax;                     // min(N, top_k): host-known bound on boxes entering NMS
-  int32_t nbmax;                    // dense mode: ceil(nmax / 64): mask layout stride
   int32_t gw, gh;                   // density grid
-  int32_t hshift;                   // Hilbert cell = 2^hshift pixels (256 x 256 cells cover the frame)
+  int32_t hshift;                   // Hilbert cell = 2^hshift pixels (128 x 128 cells cover the frame)
   int32_t lvl_start[kMaxLevels];    // first candidate of level l within the frame
   int32_t lvl_gw[kMaxLevels];       // W / s_l
-  int32_t pad_;
 };
 
 // Method constants shared by all kernels (passed by value).
@@ -36,21 +34,15 @@ struct Consts {
   float logit_thr;                  // T
   float iou_thr, iou_thr_hi, iou_thr_lo;
   int32_t iou_fast;                 // 1: the guard-banded multiply test is valid for this threshold
+  float shrink;                     // per-side shrink factor of the culling boxes: 0.49 * min(iou_thr, 1), or 0
   int32_t top_k;
+  int32_t kpad;                     // top_k rounded up to a multiple of 32: per-frame stride of the spatial arrays
   int32_t num_levels;
   int32_t stride_log2[kMaxLevels];
   int32_t cell_px;
   int32_t radius;
   float taps[2 * kMaxRadius + 1];
 };
-
-// ---- dense-mode suppression-mask layout: row-block major, upper-triangular, row-major inside a row block ----
-// word (row r, column block cb >= r/64) of a frame lives at
-//   mask_off + rb_off(rb) + (r % 64) * (nbmax - rb) + (cb - rb),  rb = r / 64
-__host__ __device__ inline int64_t mask_rb_off(int rb, int nbmax) {
-  return (int64_t)kNmsTile * ((int64_t)rb * nbmax - (int64_t)rb * (rb - 1) / 2);
-}
-__host__ __device__ inline int64_t mask_words(int nbmax) { return (int64_t)kNmsTile * nbmax * (nbmax + 1) / 2; }
 
 // ---- monotone float -> unsigned maps (descending: larger score -> smaller key) ----
 __device__ __forceinline__ uint32_t desc_key16(uint16_t h) {
@@ -63,6 +55,36 @@ __device__ __forceinline__ uint32_t desc_key32(float z) {
   if (u == 0x80000000u) u = 0;
   uint32_t asc = (u & 0x80000000u) ? ~u : (u | 0x80000000u);
   return ~asc;
+}
+
+// inverse maps: the key carries the score logit exactly (with -0 canonicalised to +0, which has the same sigmoid)
+__device__ __forceinline__ float logit_of_key16(uint32_t k16) {
+  const uint32_t asc = (~k16) & 0xFFFFu;
+  const uint16_t h = (asc & 0x8000u) ? (uint16_t)(asc & 0x7FFFu) : (uint16_t)(~asc & 0xFFFFu);
+  return __half2float(__ushort_as_half(h));
+}
+__device__ __forceinline__ float logit_of_key32(uint32_t k32) {
+  const uint32_t asc = ~k32;
+  return __uint_as_float((asc & 0x80000000u) ? (asc & 0x7FFFFFFFu) : ~asc);
+}
+template <typename KeyT> __device__ __forceinline__ int idx_of_key(KeyT key) {
+  return sizeof(KeyT) == 4 ? (int)((uint32_t)key & 0xFFFFu) : (int)(uint32_t)((uint64_t)key & 0xFFFFFFFFu);
+}
+template <typename KeyT> __device__ __forceinline__ float logit_of_key(KeyT key) {
+  return sizeof(KeyT) == 4 ? logit_of_key16((uint32_t)key >> 16) : logit_of_key32((uint32_t)((uint64_t)key >> 32));
+}
+
+// ---- culling box (DESIGN.md §6 a3) ----
+// IoU(a,b) > t implies iw > t*max(wa,wb) >= t*(wa+wb)/2 (inter = iw*ih > t*union >= t*wa*ha and ih <= ha), i.e. the boxes
+// still overlap, strictly, after each is shrunk by t/2 of its width (height) per side.  The culling boxes use
+// 0.49*t instead of 0.5*t: the 2 % slack dwarfs every fp32 rounding in this function and in the fp32 IoU of the
+// definition as long as the box is not tiny against its coordinates, which the w > 1e-3*(|x1|+|x2|) test ensures
+// (otherwise, and for NaN/inf/inverted boxes, that axis is left unshrunk, which is always conservative).
+__device__ __forceinline__ float4 shrink_box(const float4 b, const float c) {
+  const float w = __fsub_rn(b.z, b.x), h = __fsub_rn(b.w, b.y);
+  const float dx = (w > 1e-3f * (fabsf(b.x) + fabsf(b.z))) ? __fmul_rn(c, w) : 0.0f;
+  const float dy = (h > 1e-3f * (fabsf(b.y) + fabsf(b.w))) ? __fmul_rn(c, h) : 0.0f;
+  return make_float4(__fadd_rn(b.x, dx), __fadd_rn(b.y, dy), __fsub_rn(b.z, dx), __fsub_rn(b.w, dy));
 }
 
 // ---- IoU of the definition: every operation a separately rounded fp32 op ----

@@ -147,41 +147,43 @@ __global__ void __launch_bounds__(K1_THREADS) k1_threshold_compact(const uint8_t
 }
 
 // =====================================================================================================
-// a2 — segmented per-frame sort + top-K + decode + spatial order (north_star (b)).
-// One 1024-thread CTA per frame, everything after the first load in shared memory.
-//  (1) the frame's survivor keys are staged in shared memory (read once, coalesced);
-//  (2) if n > K, an MSD radix select (8-bit digits) finds the K-th smallest key — keys are unique, so exactly K
-//      keys are <= it — and an ordered in-place compaction keeps them;
-//  (3) a stable LSD block radix sort (8-bit digits, per-warp contiguous segments ranked with match_any, constant
-//      digits skipped) puts them in (score desc, index asc) order;
-//  (4) epilogue: decode the sorted rows from the raw head output (fp32, cell-centre grid point, no clipping) and
-//      write boxes / logits / candidate indices in rank order;
-//  (5) spatial order for the tiled NMS: each box gets the Hilbert index of its centre on a 256 x 256 grid, two more
-//      LSD passes sort (hilbert ‖ rank), and the boxes, their ranks and one bounding box per 32 consecutive boxes
-//      are written in that order.  The CTA also clears its frame's centroid histogram (a5).
+// Block-wide (1024-thread) helpers shared by a2 and a4: exclusive scans and a stable 8-bit LSD radix pass.
 // =====================================================================================================
-constexpr int K2_THREADS = 1024;
-constexpr int K2_WARPS = K2_THREADS / 32;
+constexpr int BLK_THREADS = 1024;
+constexpr int BLK_WARPS = BLK_THREADS / 32;
 
-template <typename KeyT> struct KeyBits { static constexpr int value = sizeof(KeyT) * 8; };
-
-// shared layout: KeyT keys[cap] | uint16 hist[32][256] | uint32 tot[256] | K2Misc
-struct K2Misc {
-  int wsum[2][K2_WARPS];
+struct BlkMisc {
+  int wsum[2][BLK_WARPS];
   int sel_digit, sel_kk, sel_tot, skip;
+  int counter;
 };
 
-__host__ __device__ inline size_t k2_smem_bytes(size_t key_slots, size_t key_bytes) {
-  return key_slots * key_bytes + K2_WARPS * 256 * sizeof(uint16_t) + 256 * sizeof(uint32_t) + sizeof(K2Misc) + 16;
+// inclusive scan of one int per thread over the CTA; returns the inclusive value, *total = sum over the CTA.
+// Two barriers; wsum row `par` is scratch (alternate rows between back-to-back calls).
+__device__ __forceinline__ int blk_scan_inclusive(int v, BlkMisc* misc, int par, int tid, int* total) {
+  const int lane = tid & 31, warp = tid >> 5;
+  int inc = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
+  if (lane == 31) misc->wsum[par][warp] = inc;
+  __syncthreads();
+  const int wv = misc->wsum[par][lane];
+  int winc = wv;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, winc, o); if (lane >= o) winc += t; }
+  const int before = __shfl_sync(0xffffffffu, winc - wv, warp);
+  *total = __shfl_sync(0xffffffffu, winc, 31);
+  __syncthreads();
+  return before + inc;
 }
 
-__device__ __forceinline__ void k2_zero_hist(uint16_t* hist, int tid) {
+__device__ __forceinline__ void blk_zero_hist(uint16_t* hist, int tid) {
   uint32_t* h32 = reinterpret_cast<uint32_t*>(hist);
-  for (int i = tid; i < K2_WARPS * 256 / 2; i += K2_THREADS) h32[i] = 0;
+  for (int i = tid; i < BLK_WARPS * 256 / 2; i += BLK_THREADS) h32[i] = 0;
 }
 
-// exclusive scan of hist in (digit major, warp minor) order, in place.  All 1024 threads.
-__device__ __forceinline__ void k2_scan_hist(uint16_t* hist, K2Misc* misc, int tid) {
+// exclusive scan of the per-warp digit histogram hist[warp][digit] in (digit major, warp minor) order, in place.
+__device__ __forceinline__ void blk_scan_hist(uint16_t* hist, BlkMisc* misc, int tid) {
   const int lane = tid & 31, warp = tid >> 5;
   const int d = tid >> 2, w0 = (tid & 3) * 8;
   int v[8], sum = 0;
@@ -204,14 +206,16 @@ __device__ __forceinline__ void k2_scan_hist(uint16_t* hist, K2Misc* misc, int t
   for (int j = 0; j < 8; ++j) { hist[(w0 + j) * 256 + d] = (uint16_t)run; run += v[j]; }
 }
 
-// One stable LSD pass on the 8-bit digit at `shift`.  Returns true if the keys moved to dst (false: digit constant).
+// One stable LSD pass on the 8-bit digit at `shift` (per-warp contiguous segments ranked with match_any).
+// Returns true if the keys moved to dst (false: the digit is constant, nothing to reorder).
 template <typename T>
-__device__ __forceinline__ bool k2_lsd_pass(const T* src, T* dst, int n, int shift, uint16_t* hist, K2Misc* misc, int tid) {
+__device__ __forceinline__ bool blk_lsd_pass(const T* src, T* dst, int n, int shift, uint16_t* hist, BlkMisc* misc, int tid) {
   const int lane = tid & 31, warp = tid >> 5;
-  const int seg = ((n + K2_WARPS - 1) / K2_WARPS + 31) & ~31;    // per-warp contiguous segment
+  const int seg = ((n + BLK_WARPS - 1) / BLK_WARPS + 31) & ~31;    // per-warp contiguous segment
   const int w_begin = warp * seg < n ? warp * seg : n;
   const int w_end = (warp + 1) * seg < n ? (warp + 1) * seg : n;
-  k2_zero_hist(hist, tid);
+  uint32_t* hist32 = reinterpret_cast<uint32_t*>(hist);
+  blk_zero_hist(hist, tid);
   if (tid == 0) misc->skip = 0;
   __syncthreads();
   for (int base = w_begin; base < w_end; base += 32) {
@@ -219,19 +223,19 @@ __device__ __forceinline__ bool k2_lsd_pass(const T* src, T* dst, int n, int shi
     const bool v = i < w_end;
     const uint32_t dg = v ? (uint32_t)((src[i] >> shift) & 255) : 256u;
     const uint32_t peers = __match_any_sync(0xffffffffu, dg);
-    if (v && lane == __ffs(peers) - 1) hist[warp * 256 + dg] += (uint16_t)__popc(peers);
-    __syncwarp();
+    // two uint16 counters per word; fire-and-forget shared atomics, no carry (a warp segment has < 65536 keys)
+    if (v && lane == __ffs(peers) - 1) atomicAdd(&hist32[(warp * 256 + dg) >> 1], (uint32_t)__popc(peers) << (16 * (dg & 1)));
   }
   __syncthreads();
   if (tid < 256) {
     int s = 0;
 #pragma unroll 8
-    for (int w = 0; w < K2_WARPS; ++w) s += hist[w * 256 + tid];
-    if (s == n) misc->skip = 1;                    // constant digit: nothing to reorder
+    for (int w = 0; w < BLK_WARPS; ++w) s += hist[w * 256 + tid];
+    if (s == n) misc->skip = 1;
   }
   __syncthreads();
   if (misc->skip) { __syncthreads(); return false; }
-  k2_scan_hist(hist, misc, tid);
+  blk_scan_hist(hist, misc, tid);
   __syncthreads();
   for (int base = w_begin; base < w_end; base += 32) {
     const int i = base + lane;
@@ -251,42 +255,67 @@ __device__ __forceinline__ bool k2_lsd_pass(const T* src, T* dst, int n, int shi
   return true;
 }
 
-// Hilbert index of cell (x, y) on a 256 x 256 grid (16 bits).  Any bijection would be correct; Hilbert order keeps 32
-// consecutive boxes in a compact connected region, which is what makes the a3 tile culling effective.
-__device__ __forceinline__ uint32_t hilbert16(uint32_t x, uint32_t y) {
+// Hilbert index of cell (x, y) on a 128 x 128 grid (14 bits).  Any bijection would be correct; Hilbert order keeps
+// consecutive boxes in a compact connected region, which is what makes the a3 block culling effective.
+__device__ __forceinline__ uint32_t hilbert14(uint32_t x, uint32_t y) {
   uint32_t d = 0;
 #pragma unroll
-  for (uint32_t s = 128; s > 0; s >>= 1) {
+  for (uint32_t s = 64; s > 0; s >>= 1) {
     const uint32_t rx = (x & s) ? 1u : 0u, ry = (y & s) ? 1u : 0u;
     d += s * s * ((3u * rx) ^ ry);
     if (ry == 0) {
-      if (rx) { x = 255u - x; y = 255u - y; }
+      if (rx) { x = 127u - x; y = 127u - y; }
       const uint32_t t = x; x = y; y = t;
     }
   }
   return d;
 }
 
+// =====================================================================================================
+// a2 — per-frame top-K selection + decode + spatial binning (north_star (b)).
+// The total order of O4 is carried by the survivor keys (descending-monotone score bits ‖ candidate index), which are
+// unique, so "the first min(n, K) of the order" is exactly the set of keys <= the K-th smallest key.  One 1024-thread
+// CTA per frame:
+//  (1) MSD radix select on 12-bit digits (3 count sweeps for 32-bit keys, early exit when a whole bucket is taken):
+//      CTA-wide counters in shared memory, warp-aggregated (match_any) fire-and-forget shared atomics, keys read
+//      straight from the L2-resident survivor list;
+//  (2) one sweep appends the keys <= threshold to shared memory (order is irrelevant from here on);
+//  (3) decode the selected rows from the raw head output (fp32, cell-centre grid point, no clipping; O1, O2) and bin
+//      each box by the Hilbert index of its centre on a 128 x 128 grid with one shared atomic (counting sort);
+//  (4) scan the 16384 bins, scatter box / culling box / key to the frame's spatial arrays, and write the bounding
+//      box of the culling boxes of every 8 and every 32 consecutive entries.
+// The (score desc, index asc) ORDER itself is applied where it is consumed: as key comparisons in a3/a4 (greedy NMS
+// only ever asks "which of two boxes comes first") and as a radix sort of the kept keys in a4, which is ~8x fewer
+// keys than sorting all top-K entries here.  The CTA also clears its frame's centroid histogram (a5).
+// =====================================================================================================
+constexpr int K2_THREADS = BLK_THREADS;
+constexpr int K2_SEL_BITS = 12;
+constexpr int K2_HBINS = 128 * 128;
+constexpr int K2_CNT_WORDS = K2_HBINS / 2;     // 32 KB: 4096 select counters (uint32) or 16384 Hilbert counters (uint16)
+
+__host__ __device__ inline size_t k2_smem_bytes(size_t top_k, size_t key_bytes) {
+  return top_k * key_bytes + top_k * sizeof(uint32_t) + K2_CNT_WORDS * sizeof(uint32_t) + sizeof(BlkMisc) + 16;
+}
+
 template <bool kHalf, typename KeyT>
-__global__ void __launch_bounds__(K2_THREADS, 1) k2_sort_topk_decode(
+__global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
     const uint8_t* __restrict__ raw, const FrameDesc* __restrict__ frames, const KeyT* __restrict__ surv_keys,
-    const int* __restrict__ surv_cnt, Consts cst, int key_slots, int nb32cap, float4* __restrict__ sorted_box,
-    float* __restrict__ sorted_logit, int* __restrict__ sorted_idx, int* __restrict__ n_sorted,
-    float4* __restrict__ sp_box, uint16_t* __restrict__ sp_rank, float4* __restrict__ bbox32,
-    uint32_t* __restrict__ hist32, int spatial) {
-  constexpr int KB = KeyBits<KeyT>::value;
+    const int* __restrict__ surv_cnt, Consts cst, int nb8cap, int nb32cap, float4* __restrict__ sel_box,
+    float4* __restrict__ sp_box, float4* __restrict__ sp_sbox, KeyT* __restrict__ sp_key, float4* __restrict__ bbox8,
+    float4* __restrict__ bbox32, int* __restrict__ n_sorted, uint32_t* __restrict__ hist32) {
+  constexpr int KB = sizeof(KeyT) * 8;
   extern __shared__ __align__(16) uint8_t smem[];
-  KeyT* keys = reinterpret_cast<KeyT*>(smem);
-  uint16_t* hist = reinterpret_cast<uint16_t*>(keys + key_slots);
-  uint32_t* tot = reinterpret_cast<uint32_t*>(hist + K2_WARPS * 256);
-  K2Misc* misc = reinterpret_cast<K2Misc*>(tot + 256);
+  const int K = cst.top_k;
+  KeyT* sel = reinterpret_cast<KeyT*>(smem);
+  uint32_t* aux = reinterpret_cast<uint32_t*>(sel + K);
+  uint32_t* cnt = aux + K;
+  BlkMisc* misc = reinterpret_cast<BlkMisc*>(cnt + K2_CNT_WORDS);
   __shared__ FrameDesc fd;
 
   const int f = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  if (tid == 0) fd = frames[f];
+  if (tid == 0) { fd = frames[f]; misc->counter = 0; }
   __syncthreads();
   const int n = surv_cnt[f];
-  const int K = cst.top_k;
   const int nsel = n < K ? n : K;
   const KeyT* gk = surv_keys + fd.cand_off;
 
@@ -297,129 +326,100 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_sort_topk_decode(
     for (int64_t i = w0 + tid; i < w1; i += K2_THREADS) hist32[i] = 0u;
   }
 
-  // ---- (1) stage ----
-  const bool staged = n <= key_slots;
-  const KeyT* all = gk;
-  if (staged) {
-    for (int i = tid; i < n; i += K2_THREADS) keys[i] = gk[i];
-    all = keys;
-    __syncthreads();
-  }
-
+  // ---- (1) threshold key = K-th smallest ----
+  KeyT thr = ~(KeyT)0;
   if (n > K) {
-    // ---- (2) MSD radix select: threshold key = K-th smallest ----
-    KeyT prefix = 0, maskbits = 0, thr = 0;
+    KeyT prefix = 0, maskbits = 0;
     int kk = K;
     bool done = false;
-    for (int shift = KB - 8; shift >= 0 && !done; shift -= 8) {
-      k2_zero_hist(hist, tid);
+    for (int hi = KB; hi > 0 && !done;) {
+      const int shift = hi > K2_SEL_BITS ? hi - K2_SEL_BITS : 0;
+      const uint32_t dmask = (1u << (hi - shift)) - 1u;
+      for (int i = tid; i < (1 << K2_SEL_BITS); i += K2_THREADS) cnt[i] = 0u;
       __syncthreads();
-      for (int base = warp * 32; base < n; base += K2_THREADS) {
-        const int i = base + lane;
-        KeyT key = 0;
-        bool m = false;
-        if (i < n) { key = all[i]; m = (key & maskbits) == prefix; }
-        const uint32_t dg = m ? (uint32_t)((key >> shift) & 255) : 256u;
-        const uint32_t peers = __match_any_sync(0xffffffffu, dg);
-        if (m && lane == __ffs(peers) - 1) hist[warp * 256 + dg] += (uint16_t)__popc(peers);
-        __syncwarp();
+      for (int base = warp * 32; base < n; base += 4 * K2_THREADS) {
+        KeyT key[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { const int i = base + u * K2_THREADS + lane; key[u] = i < n ? gk[i] : ~(KeyT)0; }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          if (base + u * K2_THREADS < n) {                      // warp-uniform
+            const int i = base + u * K2_THREADS + lane;
+            const bool m = i < n && (key[u] & maskbits) == prefix;
+            const uint32_t dg = m ? (uint32_t)((key[u] >> shift) & dmask) : 0xFFFFFFFFu;
+            const uint32_t peers = __match_any_sync(0xffffffffu, dg);
+            if (m && lane == __ffs(peers) - 1) atomicAdd(&cnt[dg], (uint32_t)__popc(peers));
+          }
+        }
       }
       __syncthreads();
-      if (tid < 256) {
-        uint32_t s = 0;
-#pragma unroll 8
-        for (int w = 0; w < K2_WARPS; ++w) s += hist[w * 256 + tid];
-        tot[tid] = s;
-      }
-      __syncthreads();
-      if (warp == 0) {
-        uint32_t v[8], s = 0;
+      {
+        uint32_t v[4];
+        int s = 0;
 #pragma unroll
-        for (int j = 0; j < 8; ++j) { v[j] = tot[lane * 8 + j]; s += v[j]; }
-        uint32_t inc = s;
+        for (int j = 0; j < 4; ++j) { v[j] = cnt[tid * 4 + j]; s += (int)v[j]; }
+        int total;
+        const int inc = blk_scan_inclusive(s, misc, 0, tid, &total);
+        int run = inc - s;                                       // keys in bins below this thread's first bin
+        if (run < kk && kk <= inc) {
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
-        uint32_t run = inc - s;                          // keys in digits below this lane's first digit
-        if (run < (uint32_t)kk && (uint32_t)kk <= inc) {
-#pragma unroll
-          for (int j = 0; j < 8; ++j) {
-            if (run < (uint32_t)kk && (uint32_t)kk <= run + v[j]) {
-              misc->sel_digit = lane * 8 + j; misc->sel_kk = kk - (int)run; misc->sel_tot = (int)v[j];
-            }
-            run += v[j];
+          for (int j = 0; j < 4; ++j) {
+            if (run < kk && kk <= run + (int)v[j]) { misc->sel_digit = tid * 4 + j; misc->sel_kk = kk - run; misc->sel_tot = (int)v[j]; }
+            run += (int)v[j];
           }
         }
       }
       __syncthreads();
       prefix |= (KeyT)misc->sel_digit << shift;
-      maskbits |= (KeyT)255 << shift;
+      maskbits |= (KeyT)dmask << shift;
       kk = misc->sel_kk;
-      if (misc->sel_tot == kk) {                          // the whole bucket is selected
+      if (misc->sel_tot == kk) {                                 // the whole bucket is selected
         thr = prefix | (shift ? (((KeyT)1 << shift) - 1) : (KeyT)0);
         done = true;
       }
+      hi = shift;
       __syncthreads();
     }
     if (!done) thr = prefix;
-    // ordered compaction of the keys <= thr into keys[0, K).  When staged it is in place: element i lands at a
-    // position <= i and every read of a 1024-chunk happens before the barrier that precedes its writes.
-    int count = 0;
-    int par = 0;
-    for (int base = 0; base < n; base += K2_THREADS, par ^= 1) {
-      const int i = base + tid;
-      KeyT key = 0;
-      bool m = false;
-      if (i < n) { key = all[i]; m = key <= thr; }
-      const uint32_t bal = __ballot_sync(0xffffffffu, m);
-      if (lane == 0) misc->wsum[par][warp] = __popc(bal);
-      __syncthreads();
-      const int wv = misc->wsum[par][lane];
-      int inc = wv;
-#pragma unroll
-      for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
-      const int before = __shfl_sync(0xffffffffu, inc - wv, warp);
-      const int total = __shfl_sync(0xffffffffu, inc, 31);
-      if (m) keys[count + before + __popc(bal & ((1u << lane) - 1u))] = key;
-      count += total;
-    }
-    __syncthreads();
-  } else if (!staged) {
-    for (int i = tid; i < n; i += K2_THREADS) keys[i] = gk[i];
-    __syncthreads();
   }
 
-  // ---- (3) stable LSD radix sort of nsel keys in shared memory ----
-  KeyT* src = keys;
-  KeyT* dst = keys + K;
-  if (nsel > 1) {
-    for (int shift = 0; shift < KB; shift += 8)
-      if (k2_lsd_pass<KeyT>(src, dst, nsel, shift, hist, misc, tid)) { KeyT* t = src; src = dst; dst = t; }
+  // ---- (2) gather the selected keys into shared memory ----
+  for (int base = warp * 32; base < n; base += K2_THREADS) {
+    const int i = base + lane;
+    KeyT key = 0;
+    bool m = false;
+    if (i < n) { key = gk[i]; m = key <= thr; }
+    const uint32_t bal = __ballot_sync(0xffffffffu, m);
+    int at = 0;
+    if (lane == 0 && bal) at = atomicAdd(&misc->counter, __popc(bal));
+    at = __shfl_sync(0xffffffffu, at, 0);
+    if (m) sel[at + __popc(bal & ((1u << lane) - 1u))] = key;
   }
+  for (int i = tid; i < K2_CNT_WORDS; i += K2_THREADS) cnt[i] = 0u;
+  __syncthreads();
 
-  // ---- (4) epilogue: decode sorted rows (O1, O2), write rank-ordered arrays, build (hilbert ‖ rank) keys ----
-  const int64_t obase = (int64_t)f * K;
-  uint32_t* mk0 = reinterpret_cast<uint32_t*>(dst);
-  uint32_t* mk1 = reinterpret_cast<uint32_t*>(src);
-  const float cmax = (float)((256 << fd.hshift) - 1);
-  for (int r = tid; r < nsel; r += K2_THREADS) {
-    const KeyT key = src[r];
-    const int idx = (sizeof(KeyT) == 4) ? (int)((uint32_t)key & 0xFFFFu) : (int)(uint32_t)(key & 0xFFFFFFFFu);
+  // ---- (3) decode (O1, O2) + Hilbert bin ----
+  const int64_t obase = (int64_t)f * cst.kpad;
+  const float cmax = (float)((128 << fd.hshift) - 1);
+  for (int i = tid; i < nsel; i += K2_THREADS) {
+    const KeyT key = sel[i];
+    const int idx = idx_of_key<KeyT>(key);
     int l = 0;
     while (l + 1 < cst.num_levels && idx >= fd.lvl_start[l + 1]) ++l;
     const int k = idx - fd.lvl_start[l];
     const int gw = fd.lvl_gw[l];
     const int iy = k / gw, ix = k - iy * gw;
     const float s = (float)(1 << cst.stride_log2[l]);
-    float v[5];
+    float v[4];
     const int64_t row = fd.cand_off + idx;
     if (kHalf) {
       const __half* p = reinterpret_cast<const __half*>(raw) + row * 5;
 #pragma unroll
-      for (int e = 0; e < 5; ++e) v[e] = __half2float(p[e]);
+      for (int e = 0; e < 4; ++e) v[e] = __half2float(p[e]);
     } else {
       const float* p = reinterpret_cast<const float*>(raw) + row * 5;
 #pragma unroll
-      for (int e = 0; e < 5; ++e) v[e] = p[e];
+      for (int e = 0; e < 4; ++e) v[e] = p[e];
     }
     const float px = __fmul_rn((float)ix + 0.5f, s), py = __fmul_rn((float)iy + 0.5f, s);
     float4 box;
@@ -427,38 +427,64 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_sort_topk_decode(
     box.y = __fsub_rn(py, __fmul_rn(v[1], s));
     box.z = __fadd_rn(px, __fmul_rn(v[2], s));
     box.w = __fadd_rn(py, __fmul_rn(v[3], s));
-    sorted_box[obase + r] = box;
-    sorted_logit[obase + r] = v[4];
-    sorted_idx[obase + r] = idx;
-    const float cx = fminf(fmaxf(0.5f * (box.x + box.z), 0.0f), cmax);
+    sel_box[obase + i] = box;
+    const float cx = fminf(fmaxf(0.5f * (box.x + box.z), 0.0f), cmax);   // NaN -> 0
     const float cy = fminf(fmaxf(0.5f * (box.y + box.w), 0.0f), cmax);
-    const uint32_t hx = (uint32_t)((int)cx >> fd.hshift), hy = (uint32_t)((int)cy >> fd.hshift);
-    mk0[r] = (hilbert16(hx, hy) << 16) | (uint32_t)r;
+    const uint32_t h = hilbert14((uint32_t)((int)cx >> fd.hshift), (uint32_t)((int)cy >> fd.hshift));
+    const uint32_t sh = 16u * (h & 1u);
+    const uint32_t old = atomicAdd(&cnt[h >> 1], 1u << sh);
+    aux[i] = (h << 16) | ((old >> sh) & 0xFFFFu);
+  }
+  __syncthreads();
+
+  // ---- (4) exclusive scan of the bins (16 per thread), scatter to spatial order ----
+  {
+    uint32_t w[8];
+    int s = 0;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) { w[j] = cnt[tid * 8 + j]; s += (int)(w[j] & 0xFFFFu) + (int)(w[j] >> 16); }
+    int total;
+    const int inc = blk_scan_inclusive(s, misc, 1, tid, &total);
+    int run = inc - s;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      const int c0 = (int)(w[j] & 0xFFFFu), c1 = (int)(w[j] >> 16);
+      cnt[tid * 8 + j] = (uint32_t)run | ((uint32_t)(run + c0) << 16);
+      run += c0 + c1;
+    }
+  }
+  __syncthreads();
+  const uint16_t* base16 = reinterpret_cast<const uint16_t*>(cnt);
+  for (int i = tid; i < nsel; i += K2_THREADS) {
+    const uint32_t a = aux[i];
+    const int pos = (int)base16[a >> 16] + (int)(a & 0xFFFFu);
+    const float4 box = sel_box[obase + i];
+    sp_box[obase + pos] = box;
+    sp_sbox[obase + pos] = shrink_box(box, cst.shrink);
+    sp_key[obase + pos] = sel[i];
+  }
+  const float inf = __int_as_float(0x7f800000);
+  const int npad = (nsel + kBlk - 1) & ~(kBlk - 1);
+  for (int i = nsel + tid; i < npad; i += K2_THREADS) {           // padding of the last block: never overlaps, never first
+    sp_sbox[obase + i] = make_float4(inf, inf, -inf, -inf);
+    sp_key[obase + i] = ~(KeyT)0;
   }
   if (tid == 0) n_sorted[f] = nsel;
   __syncthreads();
 
-  // ---- (5) spatial order ----
-  if (!spatial) return;
-  uint32_t* ms = mk0;
-  uint32_t* md = mk1;
-  if (nsel > 1) {
-    for (int shift = 16; shift < 32; shift += 8)
-      if (k2_lsd_pass<uint32_t>(ms, md, nsel, shift, hist, misc, tid)) { uint32_t* t = ms; ms = md; md = t; }
-  }
-  const float inf = __int_as_float(0x7f800000);
+  // ---- bounding boxes of the culling boxes per 8 and per 32 entries ----
   for (int s0 = warp * 32; s0 < nsel; s0 += K2_THREADS) {
-    const int s = s0 + lane;
-    float4 bb = make_float4(inf, inf, -inf, -inf);
-    if (s < nsel) {
-      const int r = (int)(ms[s] & 0xFFFFu);
-      const float4 box = sorted_box[obase + r];
-      sp_box[obase + s] = box;
-      sp_rank[obase + s] = (uint16_t)r;
-      bb = box;
-    }
+    float4 bb = sp_sbox[obase + s0 + lane];                        // padding entries are empty boxes
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
+    for (int o = 1; o < 8; o <<= 1) {
+      bb.x = fminf(bb.x, __shfl_xor_sync(0xffffffffu, bb.x, o));
+      bb.y = fminf(bb.y, __shfl_xor_sync(0xffffffffu, bb.y, o));
+      bb.z = fmaxf(bb.z, __shfl_xor_sync(0xffffffffu, bb.z, o));
+      bb.w = fmaxf(bb.w, __shfl_xor_sync(0xffffffffu, bb.w, o));
+    }
+    if ((lane & 7) == 0) bbox8[(int64_t)f * nb8cap + (s0 >> 3) + (lane >> 3)] = bb;
+#pragma unroll
+    for (int o = 8; o < 32; o <<= 1) {
       bb.x = fminf(bb.x, __shfl_xor_sync(0xffffffffu, bb.x, o));
       bb.y = fminf(bb.y, __shfl_xor_sync(0xffffffffu, bb.y, o));
       bb.z = fmaxf(bb.z, __shfl_xor_sync(0xffffffffu, bb.z, o));
@@ -469,215 +495,301 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_sort_topk_decode(
 }
 
 // =====================================================================================================
-// a3 — NMS suppression words, spatially tiled (north_star (c)).
-// The bit "box b suppresses box a" = IoU(a, b) > thr and rank(b) < rank(a) is the same bit the rank-ordered matrix
-// of the north_star sketch holds; what changes is which bits are looked at.  Boxes are in Hilbert order, 32 per block
-// (= one warp of rows, one 32-bit word of columns).  A 32 x 32 tile (row block P, column block Q) is evaluated only
-// if the blocks' bounding boxes overlap — otherwise every IoU in it is 0 and every bit is 0, exactly — and inside a
-// tile a row is skipped unless its own box overlaps Q's bounding box.  Surviving pairs take the strict-overlap
-// pre-test and then the fp32 IoU of the definition (iou_exceeds).  Each row appends its non-zero words to the row
-// block's slot range (reserved from the frame's pool with one atomicAdd per CTA): word j of a row lives at
-// W32[(slot_base[P] + j) * 32 + lane] with its column block in WQ, and nzc[row] counts them.
-// One CTA = 8 warps = 8 row blocks of one frame; the frame's block bounding boxes are staged once per CTA.
+// a3 — NMS suppression edges, spatially tiled (north_star (c)).
+// The bit "box b suppresses box a" = IoU(a, b) > thr and b before a in the order of O4 is the same bit the
+// rank-ordered matrix of the north_star sketch holds; what changes is which bits are ever looked at.  Boxes are in
+// Hilbert order.  One warp owns a block of 32 consecutive rows (lane = row); columns are visited in sub-blocks of 8.
+//  (1) block culling: the 32-row block's culling bounding box against every 32-block of the frame (ballots over the
+//      bounding boxes staged in shared memory), then each of its four 8-row groups against the four 8-column
+//      sub-blocks of every hit; all on culling boxes (boxes shrunk by ~thr/2 per side, see shrink_box), so a pair
+//      that is skipped provably has IoU <= thr.  Each group collects its own list of 8-column tiles.
+//  (2) pretest: the four groups walk their tile lists in lock step; a row tests its culling box against the tile's
+//      8 culling boxes and the order (key(b) < key(a)); 5 + 1 instructions per pair, no divergence.
+//  (3) the surviving (row, column) candidates are compacted into a per-warp queue and evaluated 32 at a time, one
+//      pair per lane, with the fp32 IoU of the definition (iou_exceeds) — full lanes on the expensive part.
+//  (4) hits are appended to the frame's edge pool as (row << 16 | column), spatial positions, via one atomicAdd per
+//      flush of the warp's staging buffer.
+// One CTA = 8 warps = 8 row blocks of one frame.
 // =====================================================================================================
 constexpr int K3_WARPS = 8;
 constexpr int K3_THREADS = 32 * K3_WARPS;
-constexpr int K3_MAX_BLOCKS = 768;              // ceil(24576 / 32)
+constexpr int K3_MAX_B32 = kMaxTopK / kBlk;     // 768
+constexpr int K3_TCAP = 32;                     // tile-list entries per 8-row group
+constexpr int K3_QCAP = 320;                    // candidate queue: <= 31 left over + <= 256 pushed per step
+constexpr int K3_SCAP = 96;                     // edge staging per warp
 
-__global__ void __launch_bounds__(K3_THREADS) k3_nms_tiles(const FrameDesc* __restrict__ frames,
+struct K3Warp {
+  float4 rowbox[kBlk];
+  uint32_t q[K3_QCAP];
+  uint32_t sb[K3_SCAP];
+  uint16_t tl[4][K3_TCAP];
+};
+
+struct K3State {                                 // warp-uniform bookkeeping
+  int qcnt, scnt;
+};
+
+__device__ __forceinline__ void k3_flush(K3Warp& W, K3State& st, const FrameDesc& fd, int f, int lane,
+                                         int* __restrict__ edge_ctr, uint32_t* __restrict__ edges,
+                                         int* __restrict__ frame_err) {
+  if (st.scnt == 0) return;
+  int base = 0;
+  if (lane == 0) base = atomicAdd(&edge_ctr[f], st.scnt);
+  base = __shfl_sync(0xffffffffu, base, 0);
+  if (base + st.scnt <= fd.edge_cap) {
+    for (int k = lane; k < st.scnt; k += 32) edges[fd.edge_off + base + k] = W.sb[k];
+  } else if (lane == 0) {
+    frame_err[f] = 1;                            // pool exhausted (only when nms_workspace_bytes was set too low)
+  }
+  st.scnt = 0;
+  __syncwarp();
+}
+
+// evaluate `nb` (<= 32) queued candidates, one per lane, from the top of the queue
+__device__ __forceinline__ void k3_exact_batch(K3Warp& W, K3State& st, int nb, const float4* __restrict__ fbox, int row0,
+                                               const Consts& cst, const FrameDesc& fd, int f, int lane,
+                                               int* __restrict__ edge_ctr, uint32_t* __restrict__ edges,
+                                               int* __restrict__ frame_err) {
+  bool hit = false;
+  uint32_t e = 0;
+  if (lane < nb) {
+    e = W.q[st.qcnt - nb + lane];
+    const float4 a = W.rowbox[e >> 16];
+    const float4 b = fbox[e & 0xFFFFu];
+    hit = iou_exceeds(a, b, cst);
+  }
+  const uint32_t bal = __ballot_sync(0xffffffffu, hit);
+  if (hit) W.sb[st.scnt + __popc(bal & ((1u << lane) - 1u))] = ((uint32_t)(row0 + (int)(e >> 16)) << 16) | (e & 0xFFFFu);
+  st.scnt += __popc(bal);
+  st.qcnt -= nb;
+  __syncwarp();
+  if (st.scnt > K3_SCAP - 32) k3_flush(W, st, fd, f, lane, edge_ctr, edges, frame_err);
+}
+
+template <typename KeyT>
+__global__ void __launch_bounds__(K3_THREADS) k3_nms_edges(const FrameDesc* __restrict__ frames,
                                                            const int* __restrict__ n_sorted,
                                                            const float4* __restrict__ sp_box,
-                                                           const uint16_t* __restrict__ sp_rank,
-                                                           const float4* __restrict__ bbox32, Consts cst, int nb32cap,
-                                                           int* __restrict__ slot_ctr, int* __restrict__ slot_base,
-                                                           uint16_t* __restrict__ nzc, uint32_t* __restrict__ W32,
-                                                           uint16_t* __restrict__ WQ, int* __restrict__ frame_err) {
-  __shared__ float4 s_bb[K3_MAX_BLOCKS];
-  __shared__ float4 s_col[K3_WARPS][kBlk];
-  __shared__ uint16_t s_cr[K3_WARPS][kBlk];
-  __shared__ int s_cnt[K3_WARPS];
-  __shared__ int s_base;
+                                                           const float4* __restrict__ sp_sbox,
+                                                           const KeyT* __restrict__ sp_key,
+                                                           const float4* __restrict__ bbox8,
+                                                           const float4* __restrict__ bbox32, Consts cst, int nb8cap,
+                                                           int nb32cap, int* __restrict__ edge_ctr,
+                                                           uint32_t* __restrict__ edges, int* __restrict__ frame_err) {
+  __shared__ float4 s_bb[K3_MAX_B32];
+  __shared__ K3Warp s_w[K3_WARPS];
+  __shared__ FrameDesc fd;
 
   const int f = blockIdx.y;
   const int n = n_sorted[f];
   if ((int)blockIdx.x * K3_THREADS >= n) return;
-  const int nb = (n + kBlk - 1) / kBlk;
+  const int nb32 = (n + kBlk - 1) / kBlk;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int64_t obase = (int64_t)f * cst.top_k;
-  const float4* fbb = bbox32 + (int64_t)f * nb32cap;
-  for (int i = tid; i < nb; i += K3_THREADS) s_bb[i] = fbb[i];
+  const int64_t obase = (int64_t)f * cst.kpad;
+  const float4* fbb32 = bbox32 + (int64_t)f * nb32cap;
+  const float4* fbb8 = bbox8 + (int64_t)f * nb8cap;
+  if (tid == 0) fd = frames[f];
+  for (int i = tid; i < nb32; i += K3_THREADS) s_bb[i] = fbb32[i];
   __syncthreads();
 
   const int P = blockIdx.x * K3_WARPS + warp;
-  const bool active = P < nb;
-  const int row = P * kBlk + lane;
-  const bool valid = active && row < n;
+  if (P >= nb32) return;
+  K3Warp& W = s_w[warp];
+  K3State st;
+  st.qcnt = 0; st.scnt = 0;
+  const float4* fbox = sp_box + obase;
+  const float4* fsbox = sp_sbox + obase;
+  const KeyT* fkey = sp_key + obase;
+  const int row0 = P * kBlk, row = row0 + lane;
   const float nanv = __int_as_float(0x7fc00000);
-  float4 a = make_float4(nanv, nanv, nanv, nanv);
-  uint32_t ra = 0;
-  if (valid) { a = sp_box[obase + row]; ra = sp_rank[obase + row]; }
-  const float4 bbP = active ? s_bb[P] : make_float4(nanv, nanv, nanv, nanv);
+  const float inf = __int_as_float(0x7f800000);
+  // rows past n are padding: culling box empty, key maximal (a2 wrote both), box NaN
+  const float4 sa = fsbox[row];
+  const KeyT keyA = fkey[row];
+  W.rowbox[lane] = row < n ? fbox[row] : make_float4(nanv, nanv, nanv, nanv);
+  const int g = lane >> 3;
+  const float4 bbP8 = fbb8[P * 4 + g];
+  const float4 bbP = s_bb[P];
+  int cnt_g = 0;                                   // entries in this lane's group's tile list (uniform within the group)
+  __syncwarp();
 
-  // neighbour blocks: word i of the bitmap lives in lane i (nb <= 768 -> <= 24 words)
-  uint32_t mybits = 0;
-  int total = 0;
-  const int nwords = (nb + 31) >> 5;
-  for (int i = 0; i < nwords; ++i) {
-    const int Q = i * 32 + lane;
-    const bool ov = Q < nb && boxes_overlap(bbP, s_bb[Q]);
-    const uint32_t b = __ballot_sync(0xffffffffu, ov);
-    if (lane == i) mybits = b;
-    total += __popc(b);
-  }
-  if (lane == 0) s_cnt[warp] = total;
-  __syncthreads();
-  if (tid == 0) {
-    int sum = 0;
+  // walk the group tile lists in lock step: pretest, queue, exact batches
+  auto drain = [&]() {
+    const int T = __reduce_max_sync(0xffffffffu, cnt_g);
+    __syncwarp();
+    for (int t = 0; t < T; ++t) {
+      uint32_t mask = 0;
+      int col0 = 0;
+      if (t < cnt_g) {
+        col0 = (int)W.tl[g][t] * kSub;
 #pragma unroll
-    for (int w = 0; w < K3_WARPS; ++w) sum += s_cnt[w];
-    const int base = atomicAdd(&slot_ctr[f], sum);
-    s_base = base;
-    if (base + sum > frames[f].slot_cap) { frame_err[f] = 1; s_base = -1; }
-  }
-  __syncthreads();
-  if (s_base < 0 || !active) return;       // pool exhausted (only when nms_workspace_bytes was set below worst case)
-  int my_base = s_base;
-  for (int w = 0; w < warp; ++w) my_base += s_cnt[w];
-  const int64_t sb = frames[f].slot_off + my_base;
-  if (lane == 0) slot_base[(int64_t)f * nb32cap + P] = (int)sb;
-
-  int nz = 0;
-  for (int i = 0; i < nwords; ++i) {
-    uint32_t bits = __shfl_sync(0xffffffffu, mybits, i);
-    while (bits) {
-      const int Q = i * 32 + __ffs(bits) - 1;
-      bits &= bits - 1;
-      const int col = Q * kBlk + lane;
-      float4 cb = make_float4(nanv, nanv, nanv, nanv);
-      uint16_t cr = 0xFFFFu;
-      if (col < n) { cb = sp_box[obase + col]; cr = sp_rank[obase + col]; }
-      __syncwarp();
-      s_col[warp][lane] = cb;
-      s_cr[warp][lane] = cr;
-      __syncwarp();
-      uint32_t word = 0;
-      if (boxes_overlap(a, s_bb[Q])) {
-#pragma unroll 8
-        for (int j = 0; j < kBlk; ++j) {
-          const float4 b = s_col[warp][j];
-          if (boxes_overlap(a, b)) {
-            if ((uint32_t)s_cr[warp][j] < ra && iou_exceeds(a, b, cst)) word |= 1u << j;
-          }
+        for (int j = 0; j < kSub; ++j) {
+          const float4 sb = fsbox[col0 + j];
+          const KeyT kb = fkey[col0 + j];
+          if (boxes_overlap(sa, sb) && kb < keyA) mask |= 1u << j;
         }
       }
-      if (word) {
-        const int64_t at = (sb + nz) * kBlk + lane;
-        W32[at] = word;
-        WQ[at] = (uint16_t)Q;
-        ++nz;
+      const int c = __popc(mask);
+      int inc = c;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
+      const int total = __shfl_sync(0xffffffffu, inc, 31);
+      if (total == 0) continue;
+      int at = st.qcnt + inc - c;
+      while (mask) {
+        const int j = __ffs(mask) - 1;
+        mask &= mask - 1;
+        W.q[at++] = ((uint32_t)lane << 16) | (uint32_t)(col0 + j);
       }
+      st.qcnt += total;
+      __syncwarp();
+      while (st.qcnt >= 32) k3_exact_batch(W, st, 32, fbox, row0, cst, fd, f, lane, edge_ctr, edges, frame_err);
+    }
+    cnt_g = 0;
+  };
+
+  const int nwords = (nb32 + 31) >> 5;
+  for (int i = 0; i < nwords; ++i) {
+    const int Q = i * 32 + lane;
+    uint32_t bits = __ballot_sync(0xffffffffu, Q < nb32 && boxes_overlap(bbP, s_bb[Q]));
+    while (bits) {
+      const int Q32 = i * 32 + __ffs(bits) - 1;
+      bits &= bits - 1;
+      // group g's 8-row box against the hit's four 8-column sub-blocks (lanes 0-3 of each group do the tests)
+      float4 bq = make_float4(inf, inf, -inf, -inf);
+      if ((lane & 4) == 0) bq = fbb8[Q32 * 4 + (lane & 3)];
+      const uint32_t b = __ballot_sync(0xffffffffu, boxes_overlap(bbP8, bq));
+      const uint32_t mine = (b >> (g * 8)) & 0xFu;
+      const int c = __popc(mine);
+      const int k = lane & 7;
+      if (k < c) {
+        uint32_t t = mine;
+        for (int z = 0; z < k; ++z) t &= t - 1;
+        W.tl[g][cnt_g + k] = (uint16_t)(Q32 * 4 + __ffs(t) - 1);
+      }
+      cnt_g += c;
+      if (__any_sync(0xffffffffu, cnt_g > K3_TCAP - 4)) drain();
     }
   }
-  if (valid) nzc[obase + row] = (uint16_t)nz;
+  drain();
+  if (st.qcnt > 0) k3_exact_batch(W, st, st.qcnt, fbox, row0, cst, fd, f, lane, edge_ctr, edges, frame_err);
+  k3_flush(W, st, fd, f, lane, edge_ctr, edges, frame_err);
 }
 
 // =====================================================================================================
-// a4 — greedy resolve + output gather + centroid histogram (north_star (c) second half; SURVEY §8(a) a4-a5,
-// §8(c) O5-O7).  One CTA per frame.  Greedy NMS in rank order is the unique solution of
-//     kept(a) <=> no b with rank(b) < rank(a), IoU(a,b) > thr is kept,
-// so instead of walking the ranks one at a time the CTA iterates to the fixed point: a pending box whose every
-// suppressor is known-removed becomes kept, one with a known-kept suppressor becomes removed.  The lowest-ranked
-// pending box always resolves, so the loop ends, and the typical depth is a handful of rounds (the longest chain of
-// overlapping boxes with decreasing score).  State is two bitmaps in shared memory (monotone, updated with atomicOr).
-// Then the kept set is mapped back to rank order, prefix-summed, and written in keep order (= score order) with the
-// sigmoid score and candidate index; each kept centroid is binned into the frame's histogram (a5).
+// a4 — greedy resolve + order + output gather + centroid histogram (north_star (c) second half; SURVEY §8(a) a4-a5,
+// §8(c) O5-O7).  One 1024-thread CTA per frame.  Greedy NMS in the order of O4 is the unique solution of
+//     kept(a)  <=>  no b before a with IoU(a,b) > thr is kept,
+// so instead of walking the order one box at a time the CTA iterates the frame's edge list (a <- b: "b, which comes
+// first, overlaps a") to the fixed point:  an edge whose b is kept removes a;  an edge whose b is removed is dropped
+// and decrements a's count of undecided suppressors;  a box whose count reaches 0 is kept.  The first undecided box
+// in the order always resolves, so the loop ends; the depth is the longest chain of overlapping boxes with
+// decreasing score (a handful of rounds).  Each thread owns a strided slice of the edge list and compacts it in
+// place, so a round only re-reads the edges that are still undecided.  State (two bitmaps, 16-bit counters) lives
+// in shared memory and is monotone.
+// Then the kept keys are radix-sorted in shared memory (this is where the (score desc, index asc) order of O4 is
+// materialised — on the kept set only), every kept box finds its output row by binary search, and is written with
+// its sigmoid score and candidate index; its centroid is binned into the frame's histogram (a5).
 // =====================================================================================================
-constexpr int K4_THREADS = 1024;
+constexpr int K4_THREADS = BLK_THREADS;
 
-__global__ void __launch_bounds__(K4_THREADS) k4_resolve_emit(
-    const FrameDesc* __restrict__ frames, const int* __restrict__ n_sorted, const float4* __restrict__ sorted_box,
-    const float* __restrict__ sorted_logit, const int* __restrict__ sorted_idx, const uint16_t* __restrict__ sp_rank,
-    const uint16_t* __restrict__ nzc, const int* __restrict__ slot_base, const uint32_t* __restrict__ W32,
-    const uint16_t* __restrict__ WQ, const int* __restrict__ frame_err, Consts cst, int nb32cap,
-    ffpp_box* __restrict__ out_boxes, int* __restrict__ out_counts, uint32_t* __restrict__ hist32) {
-  __shared__ uint32_t kept[K3_MAX_BLOCKS], removed[K3_MAX_BLOCKS], keptR[K3_MAX_BLOCKS], pref[K3_MAX_BLOCKS];
-  __shared__ int s_slot[K3_MAX_BLOCKS];
-  __shared__ int wsum[32];
+__host__ __device__ inline size_t k4_smem_bytes(size_t top_k, size_t kpad, size_t key_bytes) {
+  const size_t sort_b = 2 * top_k * key_bytes, pend_b = 2 * kpad;
+  return (sort_b > pend_b ? sort_b : pend_b) + BLK_WARPS * 256 * sizeof(uint16_t) + sizeof(BlkMisc) + 16;
+}
+
+template <typename KeyT>
+__global__ void __launch_bounds__(K4_THREADS, 1) k4_resolve_emit(
+    const FrameDesc* __restrict__ frames, const int* __restrict__ n_sorted, const float4* __restrict__ sp_box,
+    const KeyT* __restrict__ sp_key, const int* __restrict__ edge_ctr, uint32_t* __restrict__ edges,
+    const int* __restrict__ frame_err, Consts cst, ffpp_box* __restrict__ out_boxes, int* __restrict__ out_counts,
+    uint32_t* __restrict__ hist32) {
+  constexpr int KB = sizeof(KeyT) * 8;
+  extern __shared__ __align__(16) uint8_t smem[];
+  __shared__ uint32_t kept[K3_MAX_B32], removed[K3_MAX_B32];
   __shared__ FrameDesc fd;
+  const int K = cst.top_k;
+  const size_t sort_b = 2 * (size_t)K * sizeof(KeyT), pend_b = 2 * (size_t)cst.kpad;
+  uint32_t* pend = reinterpret_cast<uint32_t*>(smem);                  // two uint16 counters per word (resolve phase)
+  KeyT* list0 = reinterpret_cast<KeyT*>(smem);                         // aliases pend (sort phase)
+  KeyT* list1 = list0 + K;
+  uint16_t* hist = reinterpret_cast<uint16_t*>(smem + (sort_b > pend_b ? sort_b : pend_b));
+  BlkMisc* misc = reinterpret_cast<BlkMisc*>(hist + BLK_WARPS * 256);
+
   const int f = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   if (frame_err[f]) { if (tid == 0) out_counts[f] = -1; return; }
-  if (tid == 0) fd = frames[f];
+  if (tid == 0) { fd = frames[f]; misc->counter = 0; }
   const int n = n_sorted[f];
   const int nb = (n + kBlk - 1) / kBlk;
-  const int64_t obase = (int64_t)f * cst.top_k;
-  for (int i = tid; i < nb; i += K4_THREADS) {
-    kept[i] = 0u; removed[i] = 0u; keptR[i] = 0u;
-    s_slot[i] = slot_base[(int64_t)f * nb32cap + i];
+  const int E = edge_ctr[f];
+  const int64_t obase = (int64_t)f * cst.kpad;
+  for (int i = tid; i < nb; i += K4_THREADS) { kept[i] = 0u; removed[i] = 0u; }
+  for (int i = tid; i < (n + 1) / 2; i += K4_THREADS) pend[i] = 0u;
+  __syncthreads();
+  uint32_t* fe = edges + fd.edge_off;
+
+  // in-degrees
+  for (int e = tid; e < E; e += K4_THREADS) {
+    const uint32_t a = fe[e] >> 16;
+    atomicAdd(&pend[a >> 1], 1u << (16 * (a & 1u)));
   }
   __syncthreads();
-
-  const uint32_t bit = 1u << lane;
-  uint32_t pending = 0;
-  for (int i = 0, a = tid; a < n; ++i, a += K4_THREADS) {
-    if (nzc[obase + a] == 0) atomicOr(&kept[a >> 5], bit);
-    else pending |= 1u << i;
-  }
-  __syncthreads();
-  while (true) {
-    uint32_t m = pending;
-    while (m) {
-      const int i = __ffs(m) - 1;
-      m &= m - 1;
-      const int a = tid + i * K4_THREADS;
-      const int P = a >> 5;
-      const int c = nzc[obase + a];
-      const int64_t at = (int64_t)s_slot[P] * kBlk + lane;
-      int state = 0;                                   // 0 keep, 1 still pending, 2 remove
-      for (int j = 0; j < c; ++j) {
-        const uint32_t w = W32[at + (int64_t)j * kBlk];
-        const int Q = WQ[at + (int64_t)j * kBlk];
-        const uint32_t kq = *(volatile uint32_t*)&kept[Q];
-        const uint32_t rq = *(volatile uint32_t*)&removed[Q];
-        if (w & kq) { state = 2; break; }
-        if (w & ~rq) state = 1;
-      }
-      if (state == 2) { atomicOr(&removed[P], bit); pending &= ~(1u << i); }
-      else if (state == 0) { atomicOr(&kept[P], bit); pending &= ~(1u << i); }
-    }
-    if (!__syncthreads_or(pending != 0)) break;
-  }
-
-  // kept set -> rank order
   for (int a = tid; a < n; a += K4_THREADS)
-    if (kept[a >> 5] & bit) {
-      const uint32_t r = sp_rank[obase + a];
-      atomicOr(&keptR[r >> 5], 1u << (r & 31));
-    }
+    if (((pend[a >> 1] >> (16 * (a & 1))) & 0xFFFFu) == 0u) atomicOr(&kept[a >> 5], 1u << (a & 31));
   __syncthreads();
-  {
-    const int c = tid < nb ? __popc(keptR[tid]) : 0;
-    int inc = c;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
-    if (lane == 31) wsum[warp] = inc;
-    __syncthreads();
-    if (warp == 0) {
-      const int x = wsum[lane];
-      int xi = x;
-#pragma unroll
-      for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, xi, o); if (lane >= o) xi += t; }
-      wsum[lane] = xi - x;
-      if (lane == 31) out_counts[f] = xi;
+
+  // fixed point over this thread's strided slice of the edge list, compacted in place
+  int mine = E > tid ? (E - tid + K4_THREADS - 1) / K4_THREADS : 0;
+  const volatile uint32_t* vk = kept;
+  const volatile uint32_t* vr = removed;
+  while (true) {
+    int w = 0;
+    for (int k = 0; k < mine; ++k) {
+      const uint32_t e = fe[tid + k * K4_THREADS];
+      const uint32_t a = e >> 16, b = e & 0xFFFFu;
+      if ((vr[a >> 5] >> (a & 31)) & 1u) continue;                                  // a already removed
+      if ((vk[b >> 5] >> (b & 31)) & 1u) { atomicOr(&removed[a >> 5], 1u << (a & 31)); continue; }
+      if ((vr[b >> 5] >> (b & 31)) & 1u) {
+        const uint32_t sh = 16u * (a & 1u);
+        const uint32_t old = atomicSub(&pend[a >> 1], 1u << sh);
+        if (((old >> sh) & 0xFFFFu) == 1u) atomicOr(&kept[a >> 5], 1u << (a & 31)); // every suppressor is removed
+        continue;
+      }
+      if (w != k) fe[tid + w * K4_THREADS] = e;
+      ++w;
     }
-    __syncthreads();
-    if (tid < nb) pref[tid] = (uint32_t)(wsum[warp] + inc - c);
+    mine = w;
+    if (!__syncthreads_or(mine != 0)) break;
+  }
+
+  // kept keys -> shared list (unordered), sorted by key = keep order
+  for (int base = warp * 32; base < n; base += K4_THREADS) {
+    const int a = base + lane;
+    const bool m = a < n && ((kept[a >> 5] >> (a & 31)) & 1u);
+    const uint32_t bal = __ballot_sync(0xffffffffu, m);
+    int at = 0;
+    if (lane == 0 && bal) at = atomicAdd(&misc->counter, __popc(bal));
+    at = __shfl_sync(0xffffffffu, at, 0);
+    if (m) list0[at + __popc(bal & ((1u << lane) - 1u))] = sp_key[obase + a];
   }
   __syncthreads();
-  for (int r = tid; r < n; r += K4_THREADS) {
-    const uint32_t wd = keptR[r >> 5];
-    if (wd & bit) {
-      const int pos = (int)pref[r >> 5] + __popc(wd & (bit - 1u));
-      emit_kept(fd, cst, out_boxes + obase + pos, sorted_box[obase + r], sorted_logit[obase + r], sorted_idx[obase + r], hist32);
+  const int m = misc->counter;
+  if (tid == 0) out_counts[f] = m;
+  KeyT* src = list0;
+  KeyT* dst = list1;
+  if (m > 1) {
+    for (int shift = 0; shift < KB; shift += 8)
+      if (blk_lsd_pass<KeyT>(src, dst, m, shift, hist, misc, tid)) { KeyT* t = src; src = dst; dst = t; }
+  }
+  __syncthreads();
+
+  // emit: output row = rank of the box's key among the kept keys
+  for (int a = tid; a < n; a += K4_THREADS) {
+    if ((kept[a >> 5] >> (a & 31)) & 1u) {
+      const KeyT key = sp_key[obase + a];
+      int lo = 0, hi = m;
+      while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (src[mid] <= key) lo = mid; else hi = mid; }
+      emit_kept(fd, cst, out_boxes + (int64_t)f * K + lo, sp_box[obase + a], logit_of_key<KeyT>(key), idx_of_key<KeyT>(key), hist32);
     }
   }
 }
