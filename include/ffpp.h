@@ -54,7 +54,7 @@ typedef struct ffpp_params {
   int64_t max_total_cells; /* capacity: sum_f (W_f/cell)(H_f/cell); 0 = max_frames * (max_w/cell)(max_h/cell)       */
   int64_t nms_workspace_bytes; /* capacity of the NMS suppression-edge pool in bytes (4 per edge, shared out to the
                                   frames in proportion to min(N_f, top_k)); 0 = nms_edges_per_box edges per box       */
-  int32_t nms_edges_per_box; /* 0 = 32.  An edge is one pair (a, b) with IoU > iou_thresh, b before a in the order; the
+  int32_t nms_edges_per_box; /* 0 = 16.  An edge is one pair (a, b) with IoU > iou_thresh, b before a in the order; the
                                 flock workloads have 4-8 per box.  A frame that needs more than its share reports
                                 out_counts[f] = -1 and leaves its out_boxes / out_density rows undefined              */
   int32_t reserved_;

@@ -38,24 +38,24 @@ struct ffpp_handle {
   bool half = false;
   int key_bytes = 8;
   int kpad = 0;                       // top_k rounded up to 32: per-frame stride of the spatial arrays
-  int nb32cap = 0, nb8cap = 0;        // kpad / 32, kpad / 8
   int sm_count = 148;
   int max_frame_cand = 0;
   int64_t max_total_cells = 0;
   int64_t edge_cap_total = 0;         // suppression-edge pool, entries
-  int64_t edges_per_box = 32;
+  int64_t edges_per_box = 16;
   std::string err;
 
   // device workspace
   uint8_t* d_meta = nullptr;
   void* d_surv_keys = nullptr;
   int* d_counters = nullptr;          // 4 x max_frames: survivor counts | top-K counts | edge counters | frame_err
-  float4* d_sel_box = nullptr;        // a2 scratch: decoded boxes in selection order
+  float4* d_sel_box = nullptr;        // a2 scratch: decoded boxes in selection order; 
   float4* d_sp_box = nullptr;         // spatial (Hilbert) order, stride kpad per frame
   float4* d_sp_sbox = nullptr;        // culling boxes
   void* d_sp_key = nullptr;
-  float4* d_bbox8 = nullptr;
-  float4* d_bbox32 = nullptr;
+  uint8_t* d_hasin = nullptr;         // a3 -> a4: one byte per box, 1 = victim of at least one edge
+  uint8_t* d_k4_scratch = nullptr;    // a4 sort arrays of frames whose kept set does not fit shared memory
+  uint16_t* d_cellstart = nullptr;    // kCellStride entries per frame: start position of every spatial cell
   uint32_t* d_edges = nullptr;
   uint32_t* d_hist32 = nullptr;       // a5: uint16 count per density cell, two per word
   int64_t workspace_bytes = 0;
@@ -149,9 +149,11 @@ int schedule(ffpp_handle* h, int B, const int32_t* N, const int32_t* dims, cudaS
     d.dens_off = cells;
     d.gw = W / p.cell_px; d.gh = H / p.cell_px;
     if (d.gw < R || d.gh < R) return fail(h, FFPP_EINVAL, "density grid smaller than the Gaussian radius");
-    int hs = 0;
+    int hs = 4;                                   // 16-pixel cells unless that needs more than 128 per axis
     while ((128 << hs) < std::max(W, H)) ++hs;
     d.hshift = hs;
+    d.cgw = (W + (1 << hs) - 1) >> hs;
+    d.cgh = (H + (1 << hs) - 1) >> hs;
     d.edge_off = edges;
     d.edge_cap = (int32_t)std::min<int64_t>(h->edges_per_box * d.nmax, 0x7fffffff);
     edges += d.edge_cap;
@@ -198,23 +200,23 @@ int launch_all(ffpp_handle* h, const void* raw, int B, cudaStream_t st, ffpp_box
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[2], st));
   // a2 (+ clears the a5 histogram)
   k2_select_bin<kHalf, KeyT><<<B, K2_THREADS, k2_smem_bytes((size_t)c.top_k, sizeof(KeyT)), st>>>(
-      static_cast<const uint8_t*>(raw), frames, static_cast<const KeyT*>(h->d_surv_keys), h->surv_cnt(), c, h->nb8cap,
-      h->nb32cap, h->d_sel_box, h->d_sp_box, h->d_sp_sbox, static_cast<KeyT*>(h->d_sp_key), h->d_bbox8, h->d_bbox32,
-      h->n_sorted(), h->d_hist32);
+      static_cast<const uint8_t*>(raw), frames, static_cast<const KeyT*>(h->d_surv_keys), h->surv_cnt(), c,
+      h->d_sel_box, h->d_sp_box, h->d_sp_sbox, static_cast<KeyT*>(h->d_sp_key), h->d_cellstart, h->n_sorted(), h->d_hist32,
+      reinterpret_cast<uint32_t*>(h->d_hasin));
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[3], st));
   // a3
   {
     const dim3 g3((unsigned)((h->max_nmax + K3_THREADS - 1) / K3_THREADS), (unsigned)B);
     if (g3.x > 0)
       k3_nms_edges<KeyT><<<g3, K3_THREADS, 0, st>>>(frames, h->n_sorted(), h->d_sp_box, h->d_sp_sbox,
-                                                    static_cast<const KeyT*>(h->d_sp_key), h->d_bbox8, h->d_bbox32, c,
-                                                    h->nb8cap, h->nb32cap, h->edge_ctr(), h->d_edges, h->frame_err());
+                                                    static_cast<const KeyT*>(h->d_sp_key), h->d_cellstart, c,
+                                                    h->edge_ctr(), h->d_edges, h->d_hasin, h->frame_err());
   }
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[4], st));
   // a4 (+ a5 histogram)
   k4_resolve_emit<KeyT><<<B, K4_THREADS, k4_smem_bytes((size_t)c.top_k, (size_t)c.kpad, sizeof(KeyT)), st>>>(
-      frames, h->n_sorted(), h->d_sp_box, static_cast<const KeyT*>(h->d_sp_key), h->edge_ctr(), h->d_edges, h->frame_err(), c,
-      out_boxes, out_counts, h->d_hist32);
+      frames, h->n_sorted(), h->d_sp_box, static_cast<const KeyT*>(h->d_sp_key), h->edge_ctr(), h->d_edges,
+      reinterpret_cast<const uint32_t*>(h->d_hasin), h->frame_err(), c, h->sm_count, h->d_k4_scratch, out_boxes, out_counts, h->d_hist32);
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[5], st));
   // a6
   {
@@ -272,13 +274,11 @@ int ffpp_create(const ffpp_params* p, ffpp_handle** out) {
   h->max_frame_cand = (int)std::min<int64_t>(nmaxframe, 1 << 20);
   h->key_bytes = (h->half && nmaxframe <= 65536) ? 4 : 8;
   h->kpad = (p->top_k + kBlk - 1) / kBlk * kBlk;
-  h->nb32cap = h->kpad / kBlk;
-  h->nb8cap = h->kpad / kSub;
   {
     // shared-memory budgets of a2 (selected keys + bin bookkeeping) and a4 (two sort buffers) under the 227 KB opt-in limit
     const size_t lim = 232448;                                        // minus each kernel's static shared memory
     if (p->top_k > kMaxTopK || k2_smem_bytes((size_t)p->top_k, h->key_bytes) > lim - 512 ||
-        k4_smem_bytes((size_t)p->top_k, (size_t)h->kpad, h->key_bytes) > lim - 6656) {
+        k4_smem_bytes((size_t)p->top_k, (size_t)h->kpad, h->key_bytes) > lim - 512) {
       delete h;
       return fail(nullptr, FFPP_EINVAL, "top_k exceeds the shared-memory capacity (24576 with 32-bit keys, 12288 with 64-bit keys)");
     }
@@ -295,6 +295,12 @@ int ffpp_create(const ffpp_params* p, ffpp_handle** out) {
   c.iou_thr_hi = std::nextafterf((float)((double)p->iou_thresh * (1.0 + std::ldexp(1.0, -20))), INFINITY);
   c.iou_thr_lo = std::nextafterf((float)((double)p->iou_thresh * (1.0 - std::ldexp(1.0, -20))), -INFINITY);
   c.shrink = (p->iou_thresh >= 0.05f) ? 0.49f * std::min(p->iou_thresh, 1.0f) : 0.0f;
+  {
+    // a pair with IoU > t has |centre distance| < rho * min(w_a, w_b) per axis, rho = max(1 - t, 1/(2t) - 1/2); evaluated
+    // at a slightly smaller t (and at most 0.9) so that every fp32 rounding of the IoU of the definition is covered
+    const double te = std::min((double)p->iou_thresh, 0.9) * (1.0 - 1e-3);
+    c.rho = te >= 1e-3 ? (float)std::max(1.0 - te, 0.5 / te - 0.5) : 1e30f;
+  }
   c.top_k = p->top_k;
   c.kpad = h->kpad;
   c.num_levels = p->num_levels;
@@ -320,7 +326,7 @@ int ffpp_create(const ffpp_params* p, ffpp_handle** out) {
   const int64_t cells_frame = (int64_t)(p->max_frame_w / p->cell_px) * (p->max_frame_h / p->cell_px);
   h->max_total_cells = p->max_total_cells > 0 ? p->max_total_cells : cells_frame * p->max_frames;
   const int64_t nmax_cap = std::min<int64_t>(p->top_k, nmaxframe);
-  h->edges_per_box = p->nms_edges_per_box > 0 ? p->nms_edges_per_box : 32;
+  h->edges_per_box = p->nms_edges_per_box > 0 ? p->nms_edges_per_box : 16;
   if (p->nms_workspace_bytes > 0)
     h->edges_per_box = std::max<int64_t>(1, p->nms_workspace_bytes / 4 / (nmax_cap * p->max_frames));
   h->p.nms_edges_per_box = (int32_t)std::min<int64_t>(h->edges_per_box, 0x7fffffff);
@@ -341,8 +347,9 @@ int ffpp_create(const ffpp_params* p, ffpp_handle** out) {
       (e = dalloc((void**)&h->d_sp_box, F * KP * sizeof(float4))) != cudaSuccess ||
       (e = dalloc((void**)&h->d_sp_sbox, F * KP * sizeof(float4))) != cudaSuccess ||
       (e = dalloc(&h->d_sp_key, F * KP * (size_t)h->key_bytes)) != cudaSuccess ||
-      (e = dalloc((void**)&h->d_bbox8, F * (size_t)h->nb8cap * sizeof(float4))) != cudaSuccess ||
-      (e = dalloc((void**)&h->d_bbox32, F * (size_t)h->nb32cap * sizeof(float4))) != cudaSuccess ||
+      (e = dalloc((void**)&h->d_hasin, F * KP)) != cudaSuccess ||
+      (e = dalloc((void**)&h->d_k4_scratch, F * k4_scratch_bytes((size_t)p->top_k, (size_t)h->key_bytes))) != cudaSuccess ||
+      (e = dalloc((void**)&h->d_cellstart, F * (size_t)kCellStride * sizeof(uint16_t))) != cudaSuccess ||
       (e = dalloc((void**)&h->d_edges, (size_t)h->edge_cap_total * sizeof(uint32_t))) != cudaSuccess ||
       (e = dalloc((void**)&h->d_hist32, ((size_t)h->max_total_cells / 2 + 2) * sizeof(uint32_t))) != cudaSuccess) {
     cudaGetLastError();
@@ -426,7 +433,7 @@ int ffpp_run_host(ffpp_handle* h, const void* raw, int32_t B, const int32_t* N_p
 int ffpp_destroy(ffpp_handle* h) {
   if (!h) return FFPP_OK;
   cudaFree(h->d_meta); cudaFree(h->d_surv_keys); cudaFree(h->d_counters); cudaFree(h->d_sel_box); cudaFree(h->d_sp_box);
-  cudaFree(h->d_sp_sbox); cudaFree(h->d_sp_key); cudaFree(h->d_bbox8); cudaFree(h->d_bbox32); cudaFree(h->d_edges);
+  cudaFree(h->d_sp_sbox); cudaFree(h->d_sp_key); cudaFree(h->d_cellstart); cudaFree(h->d_hasin); cudaFree(h->d_k4_scratch); cudaFree(h->d_edges);
   cudaFree(h->d_hist32);
   cudaFree(h->d_in); cudaFree(h->d_out_boxes); cudaFree(h->d_out_counts); cudaFree(h->d_out_density);
   if (h->h_meta) cudaFreeHost(h->h_meta);
@@ -511,5 +518,13 @@ int ffpp_debug_read(ffpp_handle* h, int32_t what, void* dst, int64_t dst_bytes) 
   return FFPP_OK;
 
 }
+
+#ifdef FFPP_PROFILE_PHASES
+// development aid, compiled only with -DFFPP_PROFILE_PHASES: %globaltimer stamps of the a4 phases of the last run
+int ffpp_debug_phases(unsigned long long* dst, int frames) {
+  cudaDeviceSynchronize();
+  return (int)cudaMemcpyFromSymbol(dst, ffpp::g_phase, sizeof(unsigned long long) * 16 * (size_t)frames);
+}
+#endif
 
 }  // extern "C"

@@ -10,9 +10,10 @@ namespace ffpp {
 
 constexpr int kMaxLevels = 4;
 constexpr int kMaxRadius = 32;
-constexpr int kBlk = 32;            // boxes per spatial block = one warp of rows
-constexpr int kSub = 8;             // boxes per spatial sub-block (culling granularity of a3)
-constexpr int kMaxTopK = 24576;
+constexpr int kBlk = 32;            // kpad granularity
+constexpr int kMaxTopK = 24576;     // positions fit 15 bits (adjacency entries carry one more bit)
+constexpr int kMaxCells = 16384;    // spatial cells per frame (<= 128 x 128)
+constexpr int kCellStride = kMaxCells + 8;   // uint16 entries per frame in the cell-start table
 
 // ---- a0: frame descriptor table (device copy built by the host scheduler, one per frame) ----
 struct FrameDesc {
@@ -24,7 +25,8 @@ struct FrameDesc {
   int32_t W, H;                     // pixels
   int32_t nmax;                     // min(N, top_k): host-known bound on boxes entering NMS
   int32_t gw, gh;                   // density grid
-  int32_t hshift;                   // Hilbert cell = 2^hshift pixels (128 x 128 cells cover the frame)
+  int32_t hshift;                   // spatial cell = 2^hshift pixels
+  int32_t cgw, cgh;                 // spatial cell grid (cgw * cgh <= kMaxCells), covers [0,W) x [0,H)
   int32_t lvl_start[kMaxLevels];    // first candidate of level l within the frame
   int32_t lvl_gw[kMaxLevels];       // W / s_l
 };
@@ -35,6 +37,7 @@ struct Consts {
   float iou_thr, iou_thr_hi, iou_thr_lo;
   int32_t iou_fast;                 // 1: the guard-banded multiply test is valid for this threshold
   float shrink;                     // per-side shrink factor of the culling boxes: 0.49 * min(iou_thr, 1), or 0
+  float rho;                        // partner-centre window half-extent in units of the box's own width/height (a3)
   int32_t top_k;
   int32_t kpad;                     // top_k rounded up to a multiple of 32: per-frame stride of the spatial arrays
   int32_t num_levels;
@@ -43,6 +46,15 @@ struct Consts {
   int32_t radius;
   float taps[2 * kMaxRadius + 1];
 };
+
+// ---- development aid: per-phase %globaltimer stamps (compiled only with -DFFPP_PROFILE_PHASES) ----
+#ifdef FFPP_PROFILE_PHASES
+__device__ unsigned long long g_phase[4096][16];
+__device__ __forceinline__ unsigned long long gtimer() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+#define FFPP_PHASE(f, i) do { if (threadIdx.x == 0) g_phase[(f)][(i)] = gtimer(); } while (0)
+#else
+#define FFPP_PHASE(f, i) do { } while (0)
+#endif
 
 // ---- monotone float -> unsigned maps (descending: larger score -> smaller key) ----
 __device__ __forceinline__ uint32_t desc_key16(uint16_t h) {
@@ -85,6 +97,12 @@ __device__ __forceinline__ float4 shrink_box(const float4 b, const float c) {
   const float dx = (w > 1e-3f * (fabsf(b.x) + fabsf(b.z))) ? __fmul_rn(c, w) : 0.0f;
   const float dy = (h > 1e-3f * (fabsf(b.y) + fabsf(b.w))) ? __fmul_rn(c, h) : 0.0f;
   return make_float4(__fadd_rn(b.x, dx), __fadd_rn(b.y, dy), __fsub_rn(b.z, dx), __fsub_rn(b.w, dy));
+}
+
+// ---- spatial cells (a2 bins with these, a3 builds its windows with these: the same two functions on both sides) ----
+__device__ __forceinline__ float box_centre(const float lo, const float hi) { return __fmul_rn(0.5f, __fadd_rn(lo, hi)); }
+__device__ __forceinline__ int cell_coord(const float v, const float cmax, const int hshift) {
+  return (int)fminf(fmaxf(v, 0.0f), cmax) >> hshift;          // NaN -> 0; monotone non-decreasing in v
 }
 
 // ---- IoU of the definition: every operation a separately rounded fp32 op ----

@@ -255,22 +255,6 @@ __device__ __forceinline__ bool blk_lsd_pass(const T* src, T* dst, int n, int sh
   return true;
 }
 
-// Hilbert index of cell (x, y) on a 128 x 128 grid (14 bits).  Any bijection would be correct; Hilbert order keeps
-// consecutive boxes in a compact connected region, which is what makes the a3 block culling effective.
-__device__ __forceinline__ uint32_t hilbert14(uint32_t x, uint32_t y) {
-  uint32_t d = 0;
-#pragma unroll
-  for (uint32_t s = 64; s > 0; s >>= 1) {
-    const uint32_t rx = (x & s) ? 1u : 0u, ry = (y & s) ? 1u : 0u;
-    d += s * s * ((3u * rx) ^ ry);
-    if (ry == 0) {
-      if (rx) { x = 127u - x; y = 127u - y; }
-      const uint32_t t = x; x = y; y = t;
-    }
-  }
-  return d;
-}
-
 // =====================================================================================================
 // a2 — per-frame top-K selection + decode + spatial binning (north_star (b)).
 // The total order of O4 is carried by the survivor keys (descending-monotone score bits ‖ candidate index), which are
@@ -281,16 +265,17 @@ __device__ __forceinline__ uint32_t hilbert14(uint32_t x, uint32_t y) {
 //      straight from the L2-resident survivor list;
 //  (2) one sweep appends the keys <= threshold to shared memory (order is irrelevant from here on);
 //  (3) decode the selected rows from the raw head output (fp32, cell-centre grid point, no clipping; O1, O2) and bin
-//      each box by the Hilbert index of its centre on a 128 x 128 grid with one shared atomic (counting sort);
-//  (4) scan the 16384 bins, scatter box / culling box / key to the frame's spatial arrays, and write the bounding
-//      box of the culling boxes of every 8 and every 32 consecutive entries.
+//      each box by the spatial cell of its centre (row-major cells of 2^hshift pixels, <= 16384 per frame) with one
+//      shared atomic (counting sort);
+//  (4) scan the bins, scatter box / culling box / key to the frame's spatial arrays, and write the cell-start table
+//      (uint16 start position of every cell, row-major) that a3 uses to enumerate the boxes of a window of cells.
 // The (score desc, index asc) ORDER itself is applied where it is consumed: as key comparisons in a3/a4 (greedy NMS
 // only ever asks "which of two boxes comes first") and as a radix sort of the kept keys in a4, which is ~8x fewer
 // keys than sorting all top-K entries here.  The CTA also clears its frame's centroid histogram (a5).
 // =====================================================================================================
 constexpr int K2_THREADS = BLK_THREADS;
 constexpr int K2_SEL_BITS = 12;
-constexpr int K2_HBINS = 128 * 128;
+constexpr int K2_HBINS = kMaxCells;
 constexpr int K2_CNT_WORDS = K2_HBINS / 2;     // 32 KB: 4096 select counters (uint32) or 16384 Hilbert counters (uint16)
 
 __host__ __device__ inline size_t k2_smem_bytes(size_t top_k, size_t key_bytes) {
@@ -300,9 +285,9 @@ __host__ __device__ inline size_t k2_smem_bytes(size_t top_k, size_t key_bytes) 
 template <bool kHalf, typename KeyT>
 __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
     const uint8_t* __restrict__ raw, const FrameDesc* __restrict__ frames, const KeyT* __restrict__ surv_keys,
-    const int* __restrict__ surv_cnt, Consts cst, int nb8cap, int nb32cap, float4* __restrict__ sel_box,
-    float4* __restrict__ sp_box, float4* __restrict__ sp_sbox, KeyT* __restrict__ sp_key, float4* __restrict__ bbox8,
-    float4* __restrict__ bbox32, int* __restrict__ n_sorted, uint32_t* __restrict__ hist32) {
+    const int* __restrict__ surv_cnt, Consts cst, float4* __restrict__ sel_box, float4* __restrict__ sp_box,
+    float4* __restrict__ sp_sbox, KeyT* __restrict__ sp_key, uint16_t* __restrict__ cellstart,
+    int* __restrict__ n_sorted, uint32_t* __restrict__ hist32, uint32_t* __restrict__ hasin) {
   constexpr int KB = sizeof(KeyT) * 8;
   extern __shared__ __align__(16) uint8_t smem[];
   const int K = cst.top_k;
@@ -324,6 +309,8 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
   {
     const int64_t w0 = fd.dens_off >> 1, w1 = (fd.dens_off + (int64_t)fd.gw * fd.gh + 1) >> 1;
     for (int64_t i = w0 + tid; i < w1; i += K2_THREADS) hist32[i] = 0u;
+    uint32_t* hz = hasin + (int64_t)f * cst.kpad / 4;                   // a3's victim flags of this frame
+    for (int i = tid; i < cst.kpad / 4; i += K2_THREADS) hz[i] = 0u;
   }
 
   // ---- (1) threshold key = K-th smallest ----
@@ -398,9 +385,9 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
   for (int i = tid; i < K2_CNT_WORDS; i += K2_THREADS) cnt[i] = 0u;
   __syncthreads();
 
-  // ---- (3) decode (O1, O2) + Hilbert bin ----
+  // ---- (3) decode (O1, O2) + spatial bin ----
   const int64_t obase = (int64_t)f * cst.kpad;
-  const float cmax = (float)((128 << fd.hshift) - 1);
+  const float cmx = (float)((fd.cgw << fd.hshift) - 1), cmy = (float)((fd.cgh << fd.hshift) - 1);
   for (int i = tid; i < nsel; i += K2_THREADS) {
     const KeyT key = sel[i];
     const int idx = idx_of_key<KeyT>(key);
@@ -428,9 +415,8 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
     box.z = __fadd_rn(px, __fmul_rn(v[2], s));
     box.w = __fadd_rn(py, __fmul_rn(v[3], s));
     sel_box[obase + i] = box;
-    const float cx = fminf(fmaxf(0.5f * (box.x + box.z), 0.0f), cmax);   // NaN -> 0
-    const float cy = fminf(fmaxf(0.5f * (box.y + box.w), 0.0f), cmax);
-    const uint32_t h = hilbert14((uint32_t)((int)cx >> fd.hshift), (uint32_t)((int)cy >> fd.hshift));
+    const uint32_t h = (uint32_t)(cell_coord(box_centre(box.y, box.w), cmy, fd.hshift) * fd.cgw +
+                                  cell_coord(box_centre(box.x, box.z), cmx, fd.hshift));
     const uint32_t sh = 16u * (h & 1u);
     const uint32_t old = atomicAdd(&cnt[h >> 1], 1u << sh);
     aux[i] = (h << 16) | ((old >> sh) & 0xFFFFu);
@@ -463,108 +449,47 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
     sp_sbox[obase + pos] = shrink_box(box, cst.shrink);
     sp_key[obase + pos] = sel[i];
   }
-  const float inf = __int_as_float(0x7f800000);
-  const int npad = (nsel + kBlk - 1) & ~(kBlk - 1);
-  for (int i = nsel + tid; i < npad; i += K2_THREADS) {           // padding of the last block: never overlaps, never first
-    sp_sbox[obase + i] = make_float4(inf, inf, -inf, -inf);
-    sp_key[obase + i] = ~(KeyT)0;
-  }
-  if (tid == 0) n_sorted[f] = nsel;
-  __syncthreads();
-
-  // ---- bounding boxes of the culling boxes per 8 and per 32 entries ----
-  for (int s0 = warp * 32; s0 < nsel; s0 += K2_THREADS) {
-    float4 bb = sp_sbox[obase + s0 + lane];                        // padding entries are empty boxes
-#pragma unroll
-    for (int o = 1; o < 8; o <<= 1) {
-      bb.x = fminf(bb.x, __shfl_xor_sync(0xffffffffu, bb.x, o));
-      bb.y = fminf(bb.y, __shfl_xor_sync(0xffffffffu, bb.y, o));
-      bb.z = fmaxf(bb.z, __shfl_xor_sync(0xffffffffu, bb.z, o));
-      bb.w = fmaxf(bb.w, __shfl_xor_sync(0xffffffffu, bb.w, o));
+  // cell-start table: after the scan the counter words ARE the uint16 start positions in cell order
+  {
+    const int ncells = fd.cgw * fd.cgh;
+    uint32_t* cs32 = reinterpret_cast<uint32_t*>(cellstart + (int64_t)f * kCellStride);
+    for (int i = tid; i < (ncells + 1) / 2; i += K2_THREADS) cs32[i] = cnt[i];
+    if (tid == 0) {
+      n_sorted[f] = nsel;
+      cellstart[(int64_t)f * kCellStride + ncells] = (uint16_t)nsel;      // ncells even or odd: the terminal entry
     }
-    if ((lane & 7) == 0) bbox8[(int64_t)f * nb8cap + (s0 >> 3) + (lane >> 3)] = bb;
-#pragma unroll
-    for (int o = 8; o < 32; o <<= 1) {
-      bb.x = fminf(bb.x, __shfl_xor_sync(0xffffffffu, bb.x, o));
-      bb.y = fminf(bb.y, __shfl_xor_sync(0xffffffffu, bb.y, o));
-      bb.z = fmaxf(bb.z, __shfl_xor_sync(0xffffffffu, bb.z, o));
-      bb.w = fmaxf(bb.w, __shfl_xor_sync(0xffffffffu, bb.w, o));
-    }
-    if (lane == 0) bbox32[(int64_t)f * nb32cap + (s0 >> 5)] = bb;
   }
 }
 
 // =====================================================================================================
-// a3 — NMS suppression edges, spatially tiled (north_star (c)).
-// The bit "box b suppresses box a" = IoU(a, b) > thr and b before a in the order of O4 is the same bit the
-// rank-ordered matrix of the north_star sketch holds; what changes is which bits are ever looked at.  Boxes are in
-// Hilbert order.  One warp owns a block of 32 consecutive rows (lane = row); columns are visited in sub-blocks of 8.
-//  (1) block culling: the 32-row block's culling bounding box against every 32-block of the frame (ballots over the
-//      bounding boxes staged in shared memory), then each of its four 8-row groups against the four 8-column
-//      sub-blocks of every hit; all on culling boxes (boxes shrunk by ~thr/2 per side, see shrink_box), so a pair
-//      that is skipped provably has IoU <= thr.  Each group collects its own list of 8-column tiles.
-//  (2) pretest: the four groups walk their tile lists in lock step; a row tests its culling box against the tile's
-//      8 culling boxes and the order (key(b) < key(a)); 5 + 1 instructions per pair, no divergence.
-//  (3) the surviving (row, column) candidates are compacted into a per-warp queue and evaluated 32 at a time, one
-//      pair per lane, with the fp32 IoU of the definition (iou_exceeds) — full lanes on the expensive part.
-//  (4) hits are appended to the frame's edge pool as (row << 16 | column), spatial positions, via one atomicAdd per
-//      flush of the warp's staging buffer.
-// One CTA = 8 warps = 8 row blocks of one frame.
+// a3 — NMS suppression pairs, cell-windowed (north_star (c)).
+// The bit "IoU(a, b) > thr" is the same bit the rank-ordered matrix of the north_star sketch holds; what changes is
+// which bits are ever looked at.  Boxes are sorted by the row-major spatial cell of their centre (a2).  A pair with
+// IoU > thr has, on each axis, |centre_a - centre_b| < rho * min(w_a, w_b)  (from iw > thr * max(w_a, w_b) and
+// |dc| <= (w_a + w_b)/2 - iw;  rho = max(1 - thr, 1/(2 thr) - 1/2), DESIGN.md §6 a3), so the partner of box a lies
+// in a window of cells around a's own cell that a computes from its own size.  One thread per box; every unordered
+// pair is examined once, by the member that comes first in the spatial order: it scans the rest of its own cell row
+// and the window's rows below, each row one contiguous range of the sorted arrays, through the cell-start table.
+//  (1) pretest on the culling boxes (boxes shrunk by ~thr/2 per side, see shrink_box): 4 compares per candidate,
+//      two candidates per thread per step, all 32 threads of a warp stepping together;
+//  (2) the surviving (row, candidate) pairs are ballot-compacted into a per-warp queue and evaluated 32 at a time,
+//      one pair per lane, with the fp32 IoU of the definition (iou_exceeds) — full lanes on the expensive part;
+//  (3) a hit becomes the edge (victim << 16 | suppressor), spatial positions, the suppressor being the member that
+//      comes first in the order of O4 (smaller key); edges are staged per warp and appended to the frame's edge pool
+//      with one atomicAdd per flush, and the victim's "has a suppressor" byte is set (a plain store).
 // =====================================================================================================
 constexpr int K3_WARPS = 8;
 constexpr int K3_THREADS = 32 * K3_WARPS;
-constexpr int K3_MAX_B32 = kMaxTopK / kBlk;     // 768
-constexpr int K3_TCAP = 32;                     // tile-list entries per 8-row group
-constexpr int K3_QCAP = 320;                    // candidate queue: <= 31 left over + <= 256 pushed per step
-constexpr int K3_SCAP = 96;                     // edge staging per warp
+constexpr int K3_QCAP = 96;                     // candidate queue: <= 31 left over + <= 64 pushed per step
+constexpr int K3_SCAP = 128;                    // edge staging per warp
 
+template <typename KeyT>
 struct K3Warp {
-  float4 rowbox[kBlk];
+  float4 rowbox[32];
+  KeyT rowkey[32];
   uint32_t q[K3_QCAP];
   uint32_t sb[K3_SCAP];
-  uint16_t tl[4][K3_TCAP];
 };
-
-struct K3State {                                 // warp-uniform bookkeeping
-  int qcnt, scnt;
-};
-
-__device__ __forceinline__ void k3_flush(K3Warp& W, K3State& st, const FrameDesc& fd, int f, int lane,
-                                         int* __restrict__ edge_ctr, uint32_t* __restrict__ edges,
-                                         int* __restrict__ frame_err) {
-  if (st.scnt == 0) return;
-  int base = 0;
-  if (lane == 0) base = atomicAdd(&edge_ctr[f], st.scnt);
-  base = __shfl_sync(0xffffffffu, base, 0);
-  if (base + st.scnt <= fd.edge_cap) {
-    for (int k = lane; k < st.scnt; k += 32) edges[fd.edge_off + base + k] = W.sb[k];
-  } else if (lane == 0) {
-    frame_err[f] = 1;                            // pool exhausted (only when nms_workspace_bytes was set too low)
-  }
-  st.scnt = 0;
-  __syncwarp();
-}
-
-// evaluate `nb` (<= 32) queued candidates, one per lane, from the top of the queue
-__device__ __forceinline__ void k3_exact_batch(K3Warp& W, K3State& st, int nb, const float4* __restrict__ fbox, int row0,
-                                               const Consts& cst, const FrameDesc& fd, int f, int lane,
-                                               int* __restrict__ edge_ctr, uint32_t* __restrict__ edges,
-                                               int* __restrict__ frame_err) {
-  bool hit = false;
-  uint32_t e = 0;
-  if (lane < nb) {
-    e = W.q[st.qcnt - nb + lane];
-    const float4 a = W.rowbox[e >> 16];
-    const float4 b = fbox[e & 0xFFFFu];
-    hit = iou_exceeds(a, b, cst);
-  }
-  const uint32_t bal = __ballot_sync(0xffffffffu, hit);
-  if (hit) W.sb[st.scnt + __popc(bal & ((1u << lane) - 1u))] = ((uint32_t)(row0 + (int)(e >> 16)) << 16) | (e & 0xFFFFu);
-  st.scnt += __popc(bal);
-  st.qcnt -= nb;
-  __syncwarp();
-  if (st.scnt > K3_SCAP - 32) k3_flush(W, st, fd, f, lane, edge_ctr, edges, frame_err);
-}
 
 template <typename KeyT>
 __global__ void __launch_bounds__(K3_THREADS) k3_nms_edges(const FrameDesc* __restrict__ frames,
@@ -572,226 +497,469 @@ __global__ void __launch_bounds__(K3_THREADS) k3_nms_edges(const FrameDesc* __re
                                                            const float4* __restrict__ sp_box,
                                                            const float4* __restrict__ sp_sbox,
                                                            const KeyT* __restrict__ sp_key,
-                                                           const float4* __restrict__ bbox8,
-                                                           const float4* __restrict__ bbox32, Consts cst, int nb8cap,
-                                                           int nb32cap, int* __restrict__ edge_ctr,
-                                                           uint32_t* __restrict__ edges, int* __restrict__ frame_err) {
-  __shared__ float4 s_bb[K3_MAX_B32];
-  __shared__ K3Warp s_w[K3_WARPS];
-  __shared__ FrameDesc fd;
+                                                           const uint16_t* __restrict__ cellstart, Consts cst,
+                                                           int* __restrict__ edge_ctr, uint32_t* __restrict__ edges,
+                                                           uint8_t* __restrict__ hasin, int* __restrict__ frame_err) {
+  __shared__ K3Warp<KeyT> s_w[K3_WARPS];
 
   const int f = blockIdx.y;
   const int n = n_sorted[f];
-  if ((int)blockIdx.x * K3_THREADS >= n) return;
-  const int nb32 = (n + kBlk - 1) / kBlk;
+  const int p0 = blockIdx.x * K3_THREADS;
+  if (p0 >= n) return;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  if (p0 + warp * 32 >= n) return;
+  const FrameDesc* fd = &frames[f];
+  const int cgw = fd->cgw, cgh = fd->cgh, hs = fd->hshift;
   const int64_t obase = (int64_t)f * cst.kpad;
-  const float4* fbb32 = bbox32 + (int64_t)f * nb32cap;
-  const float4* fbb8 = bbox8 + (int64_t)f * nb8cap;
-  if (tid == 0) fd = frames[f];
-  for (int i = tid; i < nb32; i += K3_THREADS) s_bb[i] = fbb32[i];
-  __syncthreads();
-
-  const int P = blockIdx.x * K3_WARPS + warp;
-  if (P >= nb32) return;
-  K3Warp& W = s_w[warp];
-  K3State st;
-  st.qcnt = 0; st.scnt = 0;
   const float4* fbox = sp_box + obase;
   const float4* fsbox = sp_sbox + obase;
   const KeyT* fkey = sp_key + obase;
-  const int row0 = P * kBlk, row = row0 + lane;
-  const float nanv = __int_as_float(0x7fc00000);
-  const float inf = __int_as_float(0x7f800000);
-  // rows past n are padding: culling box empty, key maximal (a2 wrote both), box NaN
-  const float4 sa = fsbox[row];
-  const KeyT keyA = fkey[row];
-  W.rowbox[lane] = row < n ? fbox[row] : make_float4(nanv, nanv, nanv, nanv);
-  const int g = lane >> 3;
-  const float4 bbP8 = fbb8[P * 4 + g];
-  const float4 bbP = s_bb[P];
-  int cnt_g = 0;                                   // entries in this lane's group's tile list (uniform within the group)
+  const uint16_t* cs = cellstart + (int64_t)f * kCellStride;
+  K3Warp<KeyT>& W = s_w[warp];
+  const uint32_t lt = (1u << lane) - 1u;
+
+  const int row0 = p0 + warp * 32;
+  const int p = row0 + lane;
+  const bool valid = p < n;
+  const int pc = valid ? p : n - 1;
+  const float4 a = fbox[pc];
+  const float4 sa = fsbox[pc];
+  W.rowbox[lane] = a;
+  W.rowkey[lane] = fkey[pc];
+
+  // window of cells that can hold a partner's centre
+  const float cmx = (float)((cgw << hs) - 1), cmy = (float)((cgh << hs) - 1);
+  const float cxa = box_centre(a.x, a.z), cya = box_centre(a.y, a.w);
+  const float ex = fmaxf(cst.rho * (a.z - a.x), 0.0f) * 1.001f + 1e-5f * (fabsf(a.x) + fabsf(a.z));
+  const float ey = fmaxf(cst.rho * (a.w - a.y), 0.0f) * 1.001f + 1e-5f * (fabsf(a.y) + fabsf(a.w));
+  const int Xlo = cell_coord(cxa - ex, cmx, hs), Xhi = cell_coord(cxa + ex, cmx, hs);
+  const int Ya = cell_coord(cya, cmy, hs);
+  int Yhi = cell_coord(cya + ey, cmy, hs);
+
+  int Y = Ya, j = p + 1, e = cs[Ya * cgw + Xhi + 1];
+  if (!valid) { Y = Yhi = 0; j = e = 0; }
+  int qcnt = 0, scnt = 0;                          // warp-uniform
   __syncwarp();
 
-  // walk the group tile lists in lock step: pretest, queue, exact batches
-  auto drain = [&]() {
-    const int T = __reduce_max_sync(0xffffffffu, cnt_g);
-    __syncwarp();
-    for (int t = 0; t < T; ++t) {
-      uint32_t mask = 0;
-      int col0 = 0;
-      if (t < cnt_g) {
-        col0 = (int)W.tl[g][t] * kSub;
-#pragma unroll
-        for (int j = 0; j < kSub; ++j) {
-          const float4 sb = fsbox[col0 + j];
-          const KeyT kb = fkey[col0 + j];
-          if (boxes_overlap(sa, sb) && kb < keyA) mask |= 1u << j;
-        }
-      }
-      const int c = __popc(mask);
-      int inc = c;
-#pragma unroll
-      for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
-      const int total = __shfl_sync(0xffffffffu, inc, 31);
-      if (total == 0) continue;
-      int at = st.qcnt + inc - c;
-      while (mask) {
-        const int j = __ffs(mask) - 1;
-        mask &= mask - 1;
-        W.q[at++] = ((uint32_t)lane << 16) | (uint32_t)(col0 + j);
-      }
-      st.qcnt += total;
-      __syncwarp();
-      while (st.qcnt >= 32) k3_exact_batch(W, st, 32, fbox, row0, cst, fd, f, lane, edge_ctr, edges, frame_err);
+  auto flush = [&]() {
+    if (scnt == 0) return;
+    int base = 0;
+    if (lane == 0) base = atomicAdd(&edge_ctr[f], scnt);
+    base = __shfl_sync(0xffffffffu, base, 0);
+    if (base + scnt <= fd->edge_cap) {
+      for (int k = lane; k < scnt; k += 32) edges[fd->edge_off + base + k] = W.sb[k];
+    } else if (lane == 0) {
+      frame_err[f] = 1;                            // pool exhausted (only when nms_workspace_bytes was set too low)
     }
-    cnt_g = 0;
+    scnt = 0;
+    __syncwarp();
+  };
+  // evaluate `nb` (<= 32) queued candidates, one per lane, from the top of the queue
+  auto exact_batch = [&](const int nb) {
+    bool hit = false;
+    uint32_t ed = 0;
+    if (lane < nb) {
+      const uint32_t q = W.q[qcnt - nb + lane];
+      const uint32_t al = q >> 16, b = q & 0xFFFFu;
+      if (iou_exceeds(W.rowbox[al], fbox[b], cst)) {
+        hit = true;
+        const uint32_t pa = (uint32_t)row0 + al;
+        ed = fkey[b] < W.rowkey[al] ? ((pa << 16) | b) : ((b << 16) | pa);
+        hasin[obase + (ed >> 16)] = 1;             // a4 starts every box that is nobody's victim as kept
+      }
+    }
+    const uint32_t bal = __ballot_sync(0xffffffffu, hit);
+    if (hit) W.sb[scnt + __popc(bal & lt)] = ed;
+    scnt += __popc(bal);
+    qcnt -= nb;
+    __syncwarp();
+    if (scnt > K3_SCAP - 32) flush();
   };
 
-  const int nwords = (nb32 + 31) >> 5;
-  for (int i = 0; i < nwords; ++i) {
-    const int Q = i * 32 + lane;
-    uint32_t bits = __ballot_sync(0xffffffffu, Q < nb32 && boxes_overlap(bbP, s_bb[Q]));
-    while (bits) {
-      const int Q32 = i * 32 + __ffs(bits) - 1;
-      bits &= bits - 1;
-      // group g's 8-row box against the hit's four 8-column sub-blocks (lanes 0-3 of each group do the tests)
-      float4 bq = make_float4(inf, inf, -inf, -inf);
-      if ((lane & 4) == 0) bq = fbb8[Q32 * 4 + (lane & 3)];
-      const uint32_t b = __ballot_sync(0xffffffffu, boxes_overlap(bbP8, bq));
-      const uint32_t mine = (b >> (g * 8)) & 0xFu;
-      const int c = __popc(mine);
-      const int k = lane & 7;
-      if (k < c) {
-        uint32_t t = mine;
-        for (int z = 0; z < k; ++z) t &= t - 1;
-        W.tl[g][cnt_g + k] = (uint16_t)(Q32 * 4 + __ffs(t) - 1);
-      }
-      cnt_g += c;
-      if (__any_sync(0xffffffffu, cnt_g > K3_TCAP - 4)) drain();
+  for (;;) {
+    while (j >= e && Y < Yhi) {
+      ++Y;
+      const uint16_t* r = cs + Y * cgw;
+      j = r[Xlo];
+      e = r[Xhi + 1];
     }
+    const bool act = j < e;
+    if (!__any_sync(0xffffffffu, act)) break;
+    bool h0 = false, h1 = false;
+    if (act) {
+      const bool two = j + 1 < e;
+      const float4 sb0 = fsbox[j];
+      const float4 sb1 = fsbox[two ? j + 1 : j];
+      h0 = boxes_overlap(sa, sb0);
+      h1 = two && boxes_overlap(sa, sb1);
+    }
+    const uint32_t b0 = __ballot_sync(0xffffffffu, h0), b1 = __ballot_sync(0xffffffffu, h1);
+    if (b0 | b1) {
+      const int c0 = __popc(b0);
+      if (h0) W.q[qcnt + __popc(b0 & lt)] = ((uint32_t)lane << 16) | (uint32_t)j;
+      if (h1) W.q[qcnt + c0 + __popc(b1 & lt)] = ((uint32_t)lane << 16) | (uint32_t)(j + 1);
+      qcnt += c0 + __popc(b1);
+      __syncwarp();
+      while (qcnt >= 32) exact_batch(32);
+    }
+    j += 2;
   }
-  drain();
-  if (st.qcnt > 0) k3_exact_batch(W, st, st.qcnt, fbox, row0, cst, fd, f, lane, edge_ctr, edges, frame_err);
-  k3_flush(W, st, fd, f, lane, edge_ctr, edges, frame_err);
+  if (qcnt > 0) exact_batch(qcnt);
+  flush();
 }
 
 // =====================================================================================================
 // a4 — greedy resolve + order + output gather + centroid histogram (north_star (c) second half; SURVEY §8(a) a4-a5,
-// §8(c) O5-O7).  One 1024-thread CTA per frame.  Greedy NMS in the order of O4 is the unique solution of
+// §8(c) O5-O7).  One 512-thread CTA per frame, two CTAs per SM (296 slots: a 256-frame batch is resident at once and
+// the barriers of one frame are hidden behind the work of another).
+// Greedy NMS in the order of O4 is the unique solution of
 //     kept(a)  <=>  no b before a with IoU(a,b) > thr is kept,
-// so instead of walking the order one box at a time the CTA iterates the frame's edge list (a <- b: "b, which comes
-// first, overlaps a") to the fixed point:  an edge whose b is kept removes a;  an edge whose b is removed is dropped
-// and decrements a's count of undecided suppressors;  a box whose count reaches 0 is kept.  The first undecided box
-// in the order always resolves, so the loop ends; the depth is the longest chain of overlapping boxes with
-// decreasing score (a handful of rounds).  Each thread owns a strided slice of the edge list and compacts it in
-// place, so a round only re-reads the edges that are still undecided.  State (two bitmaps, 16-bit counters) lives
-// in shared memory and is monotone.
-// Then the kept keys are radix-sorted in shared memory (this is where the (score desc, index asc) order of O4 is
-// materialised — on the kept set only), every kept box finds its output row by binary search, and is written with
-// its sigmoid score and candidate index; its centroid is binned into the frame's histogram (a5).
+// so instead of walking the order one box at a time the CTA iterates the frame's edge list (victim <- suppressor) to
+// that fixed point, with one state byte per box in shared memory (U undecided, K kept, R removed) and two flag bytes
+// (rem, blk) — plain loads and stores, no atomics.  Boxes that are nobody's victim (a3 flagged every victim) start
+// as K; then, per round,
+//   phase 1, per edge (v <- s):  v decided -> drop;  s kept -> rem[v] = 1, drop;  s removed -> drop;
+//                                s undecided -> blk[v] = 1, keep the edge;
+//   phase 2, per box, four state bytes per 32-bit word:  U & rem -> R;  U & !rem & !blk -> K;  flags cleared.
+// The first undecided box in the order always resolves, so the loop ends; the depth is the longest chain of
+// overlapping boxes with decreasing score (a handful of rounds).  Each thread owns a strided slice of the edge list,
+// reads it eight edges at a time (the list lives in L2: memory-level parallelism, not latency, must pace the loop)
+// and compacts it in place, so a round only re-reads the edges that are still undecided.
+// Then the kept boxes are ordered: their keys and spatial positions are gathered through a prefix sum of the kept
+// bitmap and sorted by key with a bitonic network (this is where the (score desc, index asc) order of O4 is
+// materialised — on the kept set only); output row r is the r-th pair, written with its sigmoid score and
+// candidate index, and its centroid is binned into the frame's histogram (a5).  The sort arrays live in shared
+// memory when the kept count (rounded up to a power of two) fits, else in a global scratch area.
 // =====================================================================================================
-constexpr int K4_THREADS = BLK_THREADS;
+constexpr int K4_THREADS = 512;
+constexpr int K4_WARPS = K4_THREADS / 32;
+constexpr int K4_SMEM_BUDGET = 108 * 1024;       // dynamic shared memory per CTA (two CTAs per SM)
+constexpr int K4_MAXPERM = 1024;                 // batches up to this many frames get the weight-ordered CTA -> frame map
+constexpr int K4_UNROLL = 8;
+constexpr int K4_BITONIC_MAX = 1024;             // kept sets up to this size take the bitonic network, larger ones LSD radix
+constexpr uint32_t ST_U = 0, ST_K = 1, ST_R = 2;
 
+struct K4Misc {
+  int wsum[K4_WARPS];
+};
+
+__host__ __device__ inline size_t k4_pow2ceil(size_t v) { size_t p = 1; while (p < v) p <<= 1; return p; }
+// bytes of the resolve/sort union region and of the fixed tail (kept bitmap, its word prefix, misc)
+__host__ __device__ inline size_t k4_tail_bytes(size_t kpad) {
+  return kpad / 8 + ((kpad / 32 * 2 + 15) & ~(size_t)15) + K4_WARPS * 256 * sizeof(uint16_t) + sizeof(K4Misc) + 16;
+}
+// sort arrays for m kept boxes: two (key, position) buffers, m rounded up to a power of two for the bitonic path
+__host__ __device__ inline size_t k4_sort_bytes(size_t m, size_t key_bytes) {
+  const size_t lsd = 2 * (((m * key_bytes + 15) & ~(size_t)15) + ((m * 2 + 15) & ~(size_t)15));
+  const size_t bit = m <= (size_t)K4_BITONIC_MAX ? k4_pow2ceil(m) * (key_bytes + 2) : 0;
+  return lsd > bit ? lsd : bit;
+}
+__host__ __device__ inline size_t k4_union_bytes(size_t top_k, size_t kpad, size_t key_bytes) {
+  const size_t flag_b = 3 * kpad;
+  size_t sort_b = k4_sort_bytes(top_k, key_bytes);
+  const size_t room = (size_t)K4_SMEM_BUDGET - k4_tail_bytes(kpad);
+  if (sort_b > room) sort_b = room;
+  return ((sort_b > flag_b ? sort_b : flag_b) + 15) & ~(size_t)15;
+}
 __host__ __device__ inline size_t k4_smem_bytes(size_t top_k, size_t kpad, size_t key_bytes) {
-  const size_t sort_b = 2 * top_k * key_bytes, pend_b = 2 * kpad;
-  return (sort_b > pend_b ? sort_b : pend_b) + BLK_WARPS * 256 * sizeof(uint16_t) + sizeof(BlkMisc) + 16;
+  return k4_union_bytes(top_k, kpad, key_bytes) + k4_tail_bytes(kpad);
+}
+__host__ __device__ inline size_t k4_scratch_bytes(size_t top_k, size_t key_bytes) {   // per frame
+  return (k4_sort_bytes(top_k, key_bytes) + 15) & ~(size_t)15;
+}
+
+// lanes of the warp that hold the same 8-bit digit (ballot per digit bit: a fixed 8 steps whatever the digit mix)
+__device__ __forceinline__ uint32_t k4_peers8(const uint32_t dg, const bool v) {
+  uint32_t p = __ballot_sync(0xffffffffu, v);
+#pragma unroll
+  for (int b = 0; b < 8; ++b) {
+    const bool bit = (dg >> b) & 1u;
+    const uint32_t bal = __ballot_sync(0xffffffffu, bit);
+    p &= bit ? bal : ~bal;
+  }
+  return p;
+}
+
+// One stable LSD pass (8-bit digit at `shift`) over m (key, position) pairs, 512 threads.  Returns false (nothing
+// moved) when the digit is the same for every key.  hist = 16 warps x 256 digits.
+template <typename KeyT>
+__device__ __forceinline__ bool k4_lsd_pass(const KeyT* ksrc, const uint16_t* psrc, KeyT* kdst, uint16_t* pdst, int m,
+                                            int shift, uint16_t* hist, K4Misc* misc, int tid) {
+  const int lane = tid & 31, warp = tid >> 5;
+  const int seg = ((m + K4_WARPS - 1) / K4_WARPS + 31) & ~31;      // per-warp contiguous segment
+  const int w_begin = warp * seg < m ? warp * seg : m;
+  const int w_end = (warp + 1) * seg < m ? (warp + 1) * seg : m;
+  uint32_t* hist32 = reinterpret_cast<uint32_t*>(hist);
+  for (int i = tid; i < K4_WARPS * 256 / 2; i += K4_THREADS) hist32[i] = 0u;
+  __syncthreads();
+  for (int base = w_begin; base < w_end; base += 32) {
+    const int i = base + lane;
+    const bool v = i < w_end;
+    const uint32_t dg = v ? (uint32_t)((ksrc[i] >> shift) & 255) : 0u;
+    const uint32_t peers = k4_peers8(dg, v);
+    // two uint16 counters per word; no carry (a warp segment has < 65536 entries)
+    if (v && lane == __ffs(peers) - 1) atomicAdd(&hist32[(warp * 256 + dg) >> 1], (uint32_t)__popc(peers) << (16 * (dg & 1)));
+  }
+  __syncthreads();
+  // thread d < 256 owns digit d: counts of the 16 warps, exclusive offsets in (digit major, warp minor) order
+  int c[K4_WARPS], s = 0;
+  if (tid < 256) {
+#pragma unroll
+    for (int w = 0; w < K4_WARPS; ++w) { c[w] = hist[w * 256 + tid]; s += c[w]; }
+  }
+  if (__syncthreads_or(s == m)) return false;
+  int inc = s;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
+  if (lane == 31) misc->wsum[warp] = inc;
+  __syncthreads();
+  if (tid < 256) {
+    int run = inc - s;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) if (w < warp) run += misc->wsum[w];
+#pragma unroll
+    for (int w = 0; w < K4_WARPS; ++w) { hist[w * 256 + tid] = (uint16_t)run; run += c[w]; }
+  }
+  __syncthreads();
+  for (int base = w_begin; base < w_end; base += 32) {
+    const int i = base + lane;
+    const bool v = i < w_end;
+    KeyT key = 0;
+    uint16_t pe = 0;
+    if (v) { key = ksrc[i]; pe = psrc[i]; }
+    const uint32_t dg = v ? (uint32_t)((key >> shift) & 255) : 0u;
+    const uint32_t peers = k4_peers8(dg, v);
+    int b = 0;
+    if (v) b = hist[warp * 256 + dg];
+    __syncwarp();
+    if (v && lane == __ffs(peers) - 1) hist[warp * 256 + dg] = (uint16_t)(b + __popc(peers));
+    __syncwarp();
+    if (v) { const int o = b + __popc(peers & ((1u << lane) - 1u)); kdst[o] = key; pdst[o] = pe; }
+  }
+  __syncthreads();
+  return true;
 }
 
 template <typename KeyT>
-__global__ void __launch_bounds__(K4_THREADS, 1) k4_resolve_emit(
+__global__ void __launch_bounds__(K4_THREADS, 2) k4_resolve_emit(
     const FrameDesc* __restrict__ frames, const int* __restrict__ n_sorted, const float4* __restrict__ sp_box,
-    const KeyT* __restrict__ sp_key, const int* __restrict__ edge_ctr, uint32_t* __restrict__ edges,
-    const int* __restrict__ frame_err, Consts cst, ffpp_box* __restrict__ out_boxes, int* __restrict__ out_counts,
-    uint32_t* __restrict__ hist32) {
-  constexpr int KB = sizeof(KeyT) * 8;
+    const KeyT* __restrict__ sp_key, const int* __restrict__ edge_ctr, uint32_t* edges,
+    const uint32_t* __restrict__ hasin, const int* __restrict__ frame_err, Consts cst, int sm_count, uint8_t* __restrict__ scratch,
+    ffpp_box* __restrict__ out_boxes, int* __restrict__ out_counts, uint32_t* __restrict__ hist32) {
   extern __shared__ __align__(16) uint8_t smem[];
-  __shared__ uint32_t kept[K3_MAX_B32], removed[K3_MAX_B32];
   __shared__ FrameDesc fd;
-  const int K = cst.top_k;
-  const size_t sort_b = 2 * (size_t)K * sizeof(KeyT), pend_b = 2 * (size_t)cst.kpad;
-  uint32_t* pend = reinterpret_cast<uint32_t*>(smem);                  // two uint16 counters per word (resolve phase)
-  KeyT* list0 = reinterpret_cast<KeyT*>(smem);                         // aliases pend (sort phase)
-  KeyT* list1 = list0 + K;
-  uint16_t* hist = reinterpret_cast<uint16_t*>(smem + (sort_b > pend_b ? sort_b : pend_b));
-  BlkMisc* misc = reinterpret_cast<BlkMisc*>(hist + BLK_WARPS * 256);
+  const int K = cst.top_k, kpad = cst.kpad;
+  const size_t uni_b = k4_union_bytes((size_t)K, (size_t)kpad, sizeof(KeyT));
+  uint32_t* st32 = reinterpret_cast<uint32_t*>(smem);                  // resolve phase: state, rem, blk bytes
+  uint32_t* rem32 = reinterpret_cast<uint32_t*>(smem + kpad);
+  uint32_t* blk32 = reinterpret_cast<uint32_t*>(smem + 2 * kpad);
+  uint8_t* st = smem;
+  uint8_t* rem = smem + kpad;
+  uint8_t* blk = smem + 2 * kpad;
+  uint32_t* keptw = reinterpret_cast<uint32_t*>(smem + uni_b);         // kept bitmap, kpad / 32 words
+  uint16_t* wpre = reinterpret_cast<uint16_t*>(smem + uni_b + kpad / 8);   // kept boxes before each bitmap word
+  uint16_t* hist = reinterpret_cast<uint16_t*>(smem + uni_b + kpad / 8 + ((kpad / 32 * 2 + 15) & ~15));
+  K4Misc* misc = reinterpret_cast<K4Misc*>(hist + K4_WARPS * 256);
 
-  const int f = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  // Which frame this CTA takes.  All CTAs start at once, two per SM, and the hardware hands out CTAs 0..S-1 one per
+  // SM before it doubles up: give those the S heaviest frames (heaviest first) and pair them with the lightest ones.
+  __shared__ int s_w[K4_MAXPERM];
+  __shared__ int s_frame;
+  {
+    const int B = (int)gridDim.x, S = sm_count, i = (int)blockIdx.x;
+    if (B <= S || B > K4_MAXPERM) {
+      if (tid == 0) s_frame = i;
+    } else {
+      for (int g = tid; g < B; g += K4_THREADS) s_w[g] = edge_ctr[g] + 3 * n_sorted[g];
+      __syncthreads();
+      const int want = i < S ? i : (i < 2 * S ? B - 1 - (i - S) : S + (i - 2 * S));     // rank in descending weight
+      for (int g = tid; g < B; g += K4_THREADS) {
+        const int wg = s_w[g];
+        int rank = 0;
+        for (int h = 0; h < B; ++h) { const int wh = s_w[h]; rank += (wh > wg) | ((wh == wg) & (h < g)); }
+        if (rank == want) s_frame = g;
+      }
+    }
+    __syncthreads();
+  }
+  const int f = s_frame;
   if (frame_err[f]) { if (tid == 0) out_counts[f] = -1; return; }
-  if (tid == 0) { fd = frames[f]; misc->counter = 0; }
+  FFPP_PHASE(f, 0);
+  if (tid == 0) fd = frames[f];
   const int n = n_sorted[f];
-  const int nb = (n + kBlk - 1) / kBlk;
-  const int E = edge_ctr[f];
-  const int64_t obase = (int64_t)f * cst.kpad;
-  for (int i = tid; i < nb; i += K4_THREADS) { kept[i] = 0u; removed[i] = 0u; }
-  for (int i = tid; i < (n + 1) / 2; i += K4_THREADS) pend[i] = 0u;
+  const int64_t obase = (int64_t)f * kpad;
+  {
+    const uint32_t* hin = hasin + obase / 4;
+    for (int i = tid; i < kpad / 4; i += K4_THREADS) {
+      st32[i] = hin[i] ^ 0x01010101u;                                  // victim of some edge -> U, else K
+      rem32[i] = 0u;
+      blk32[i] = 0u;
+    }
+  }
   __syncthreads();
+  FFPP_PHASE(f, 1);
+  const int E = edge_ctr[f];
   uint32_t* fe = edges + fd.edge_off;
 
-  // in-degrees
-  for (int e = tid; e < E; e += K4_THREADS) {
-    const uint32_t a = fe[e] >> 16;
-    atomicAdd(&pend[a >> 1], 1u << (16 * (a & 1u)));
-  }
-  __syncthreads();
-  for (int a = tid; a < n; a += K4_THREADS)
-    if (((pend[a >> 1] >> (16 * (a & 1))) & 0xFFFFu) == 0u) atomicOr(&kept[a >> 5], 1u << (a & 31));
-  __syncthreads();
-
-  // fixed point over this thread's strided slice of the edge list, compacted in place
+  // ---- fixed point over this thread's strided slice of the edge list, compacted in place ----
   int mine = E > tid ? (E - tid + K4_THREADS - 1) / K4_THREADS : 0;
-  const volatile uint32_t* vk = kept;
-  const volatile uint32_t* vr = removed;
-  while (true) {
+  const int nw = (n + 3) >> 2;
+#ifdef FFPP_PROFILE_PHASES
+  int round_ = 0;
+#endif
+  bool first = true;                       // round 1 drops nothing: every victim is still U, so it only sets flags
+  for (;;) {
     int w = 0;
-    for (int k = 0; k < mine; ++k) {
-      const uint32_t e = fe[tid + k * K4_THREADS];
-      const uint32_t a = e >> 16, b = e & 0xFFFFu;
-      if ((vr[a >> 5] >> (a & 31)) & 1u) continue;                                  // a already removed
-      if ((vk[b >> 5] >> (b & 31)) & 1u) { atomicOr(&removed[a >> 5], 1u << (a & 31)); continue; }
-      if ((vr[b >> 5] >> (b & 31)) & 1u) {
-        const uint32_t sh = 16u * (a & 1u);
-        const uint32_t old = atomicSub(&pend[a >> 1], 1u << sh);
-        if (((old >> sh) & 0xFFFFu) == 1u) atomicOr(&kept[a >> 5], 1u << (a & 31)); // every suppressor is removed
-        continue;
+    uint32_t nx[K4_UNROLL];
+#pragma unroll
+    for (int u = 0; u < K4_UNROLL; ++u) nx[u] = u < mine ? fe[tid + u * K4_THREADS] : 0u;
+    for (int k0 = 0; k0 < mine; k0 += K4_UNROLL) {
+      uint32_t ed[K4_UNROLL], sv[K4_UNROLL], ss[K4_UNROLL];
+#pragma unroll
+      for (int u = 0; u < K4_UNROLL; ++u) ed[u] = nx[u];
+#pragma unroll
+      for (int u = 0; u < K4_UNROLL; ++u)     // next batch: slots beyond anything this batch can write
+        nx[u] = k0 + K4_UNROLL + u < mine ? fe[tid + (k0 + K4_UNROLL + u) * K4_THREADS] : 0u;
+#pragma unroll
+      for (int u = 0; u < K4_UNROLL; ++u) { sv[u] = st[ed[u] >> 16]; ss[u] = st[ed[u] & 0xFFFFu]; }
+#pragma unroll
+      for (int u = 0; u < K4_UNROLL; ++u) {
+        if (k0 + u < mine && sv[u] == ST_U) {
+          const uint32_t v = ed[u] >> 16;
+          if (ss[u] == ST_K) {
+            rem[v] = 1;
+          } else if (ss[u] == ST_U) {
+            blk[v] = 1;
+            if (!first) { fe[tid + w * K4_THREADS] = ed[u]; ++w; }
+          }
+        }
       }
-      if (w != k) fe[tid + w * K4_THREADS] = e;
-      ++w;
     }
-    mine = w;
+    if (!first) mine = w;
+    first = false;
+    __syncthreads();
+    for (int i = tid; i < nw; i += K4_THREADS) {
+      const uint32_t s4 = st32[i], r4 = rem32[i], b4 = blk32[i];
+      const uint32_t isu = ((s4 | (s4 >> 1)) & 0x01010101u) ^ 0x01010101u;          // 1 in every byte that is U
+      const uint32_t val = (r4 << 1) | ((r4 | b4) ^ 0x01010101u);                   // R if rem, K if neither, U if blk only
+      st32[i] = s4 | (val & (isu | (isu << 1)));
+      rem32[i] = 0u;
+      blk32[i] = 0u;
+    }
+#ifdef FFPP_PROFILE_PHASES
+    if (round_ < 8) FFPP_PHASE(f, 8 + round_);
+    ++round_;
+#endif
     if (!__syncthreads_or(mine != 0)) break;
   }
+  FFPP_PHASE(f, 2);
 
-  // kept keys -> shared list (unordered), sorted by key = keep order
-  for (int base = warp * 32; base < n; base += K4_THREADS) {
+  // ---- kept bitmap + its word prefix (the state bytes are about to be overwritten by the sort arrays) ----
+  const int nwords = kpad / 32;
+  for (int base = warp * 32; base < kpad; base += K4_THREADS) {
     const int a = base + lane;
-    const bool m = a < n && ((kept[a >> 5] >> (a & 31)) & 1u);
-    const uint32_t bal = __ballot_sync(0xffffffffu, m);
-    int at = 0;
-    if (lane == 0 && bal) at = atomicAdd(&misc->counter, __popc(bal));
-    at = __shfl_sync(0xffffffffu, at, 0);
-    if (m) list0[at + __popc(bal & ((1u << lane) - 1u))] = sp_key[obase + a];
+    const uint32_t bal = __ballot_sync(0xffffffffu, a < n && st[a] == ST_K);
+    if (lane == 0) keptw[base >> 5] = bal;
   }
   __syncthreads();
-  const int m = misc->counter;
+  int m = 0;
+  {
+    // each thread owns a contiguous run of words; block-wide exclusive scan of the runs' popcounts
+    const int per = (nwords + K4_THREADS - 1) / K4_THREADS;
+    const int w0 = tid * per, w1 = w0 + per < nwords ? w0 + per : nwords;
+    int s = 0;
+    for (int i = w0; i < w1; ++i) s += __popc(keptw[i]);
+    int inc = s;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
+    if (lane == 31) misc->wsum[warp] = inc;
+    __syncthreads();
+    int run = inc - s;
+#pragma unroll
+    for (int w = 0; w < K4_WARPS; ++w) { const int ws = misc->wsum[w]; if (w < warp) run += ws; m += ws; }
+    for (int i = w0; i < w1; ++i) { wpre[i] = (uint16_t)run; run += __popc(keptw[i]); }
+  }
   if (tid == 0) out_counts[f] = m;
-  KeyT* src = list0;
-  KeyT* dst = list1;
-  if (m > 1) {
-    for (int shift = 0; shift < KB; shift += 8)
-      if (blk_lsd_pass<KeyT>(src, dst, m, shift, hist, misc, tid)) { KeyT* t = src; src = dst; dst = t; }
-  }
   __syncthreads();
+  FFPP_PHASE(f, 3);
 
-  // emit: output row = rank of the box's key among the kept keys
-  for (int a = tid; a < n; a += K4_THREADS) {
-    if ((kept[a >> 5] >> (a & 31)) & 1u) {
-      const KeyT key = sp_key[obase + a];
-      int lo = 0, hi = m;
-      while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (src[mid] <= key) lo = mid; else hi = mid; }
-      emit_kept(fd, cst, out_boxes + (int64_t)f * K + lo, sp_box[obase + a], logit_of_key<KeyT>(key), idx_of_key<KeyT>(key), hist32);
+  // ---- sort arrays: (key, position) pairs; bitonic network for small sets, LSD radix beyond ----
+  constexpr int KB = sizeof(KeyT) * 8;
+  const bool bitonic = m <= K4_BITONIC_MAX;
+  const int Np = bitonic ? (int)k4_pow2ceil((size_t)(m > 1 ? m : 1)) : m;
+  uint8_t* lbase = k4_sort_bytes((size_t)m, sizeof(KeyT)) <= uni_b ? smem : scratch + (size_t)f * k4_scratch_bytes((size_t)K, sizeof(KeyT));
+  const size_t kbytes = ((size_t)Np * sizeof(KeyT) + 15) & ~(size_t)15, pbytes = ((size_t)Np * 2 + 15) & ~(size_t)15;
+  KeyT* kk = reinterpret_cast<KeyT*>(lbase);
+  uint16_t* pp = reinterpret_cast<uint16_t*>(lbase + kbytes);
+  KeyT* kk1 = reinterpret_cast<KeyT*>(lbase + kbytes + pbytes);          // second buffer (LSD path only)
+  uint16_t* pp1 = reinterpret_cast<uint16_t*>(lbase + 2 * kbytes + pbytes);
+  for (int base0 = warp * 32; base0 < n; base0 += 4 * K4_THREADS) {
+    KeyT key[4];
+    uint32_t bal[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int base = base0 + u * K4_THREADS;
+      bal[u] = base < n ? keptw[base >> 5] : 0u;
+      if ((bal[u] >> lane) & 1u) key[u] = sp_key[obase + base + lane];
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int base = base0 + u * K4_THREADS;
+      if ((bal[u] >> lane) & 1u) {
+        const int i = (int)wpre[base >> 5] + __popc(bal[u] & ((1u << lane) - 1u));
+        kk[i] = key[u];
+        pp[i] = (uint16_t)(base + lane);
+      }
     }
   }
+  if (bitonic)
+    for (int i = m + tid; i < Np; i += K4_THREADS) { kk[i] = ~(KeyT)0; pp[i] = 0; }
+  __syncthreads();
+  FFPP_PHASE(f, 4);
+  if (bitonic) {
+    for (int k = 2; k <= Np; k <<= 1) {
+      for (int j = k >> 1; j > 0; j >>= 1) {
+        for (int t = tid; t < (Np >> 1); t += K4_THREADS) {
+          const int i = ((t & ~(j - 1)) << 1) | (t & (j - 1)), l = i | j;
+          const KeyT ka = kk[i], kb = kk[l];
+          if ((ka > kb) == ((i & k) == 0)) {
+            kk[i] = kb; kk[l] = ka;
+            const uint16_t t0 = pp[i]; pp[i] = pp[l]; pp[l] = t0;
+          }
+        }
+        __syncthreads();
+      }
+    }
+  } else {
+    for (int shift = 0; shift < KB; shift += 8)
+      if (k4_lsd_pass<KeyT>(kk, pp, kk1, pp1, m, shift, hist, misc, tid)) {
+        KeyT* tk = kk; kk = kk1; kk1 = tk;
+        uint16_t* tp = pp; pp = pp1; pp1 = tp;
+      }
+  }
+  FFPP_PHASE(f, 5);
+
+  // ---- emit: output row r = r-th kept box in key order ----
+  for (int r0 = tid; r0 < m; r0 += 4 * K4_THREADS) {
+    KeyT key[4];
+    float4 bx[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int r = r0 + u * K4_THREADS;
+      if (r < m) { key[u] = kk[r]; bx[u] = sp_box[obase + pp[r]]; }
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int r = r0 + u * K4_THREADS;
+      if (r < m) emit_kept(fd, cst, out_boxes + (int64_t)f * K + r, bx[u], logit_of_key<KeyT>(key[u]), idx_of_key<KeyT>(key[u]), hist32);
+    }
+  }
+#ifdef FFPP_PROFILE_PHASES
+  __syncthreads();
+  FFPP_PHASE(f, 6);
+  if (tid == 0) g_phase[f][7] = ((unsigned long long)n << 40) | ((unsigned long long)E << 16) | (unsigned long long)m;
+#endif
 }
 
 // =====================================================================================================
