@@ -12,6 +12,10 @@
 
 using namespace ffpp;
 
+// compile-time radii of the a6 kernel; a run uses the smallest one >= floor(truncate * sigma)
+#define FFPP_K5_RADII(X) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(12) X(14) X(16) X(20) X(24) X(28) X(32)
+#define FFPP_K5_LIST(RT) RT,
+
 namespace {
 
 thread_local std::string g_create_error;
@@ -160,7 +164,7 @@ int schedule(ffpp_handle* h, int B, const int32_t* N, const int32_t* dims, cudaS
     fr[f] = d;
     coff[f] = cand;
     cand += n; cells += (int64_t)d.gw * d.gh;
-    const int tiles = ((d.gw + K5_TW - 1) / K5_TW) * ((d.gh + K5_TH - 1) / K5_TH);
+    const int tiles = k5_tiles(d.gw, d.gh);
     max_tiles = std::max(max_tiles, tiles);
     max_nmax = std::max(max_nmax, (int)d.nmax);
   }
@@ -221,8 +225,14 @@ int launch_all(ffpp_handle* h, const void* raw, int B, cudaStream_t st, ffpp_box
   // a6
   {
     const dim3 g5((unsigned)h->max_tiles, (unsigned)B);
-    k5_density<<<g5, K5_THREADS, k5_smem_bytes(c.radius), st>>>(frames, c, reinterpret_cast<const uint16_t*>(h->d_hist32),
-                                                                 out_density);
+    const size_t s5 = k5_smem_bytes(h->p.max_frame_w / h->p.cell_px, c.radius_t);
+    const uint16_t* h16 = reinterpret_cast<const uint16_t*>(h->d_hist32);
+    switch (c.radius_t) {
+#define FFPP_K5_CASE(RT) case RT: k5_density<RT><<<g5, K5_THREADS, s5, st>>>(frames, c, h16, out_density); break;
+      FFPP_K5_RADII(FFPP_K5_CASE)
+#undef FFPP_K5_CASE
+      default: return fail(h, FFPP_EINVAL, "no a6 kernel for this radius");
+    }
   }
   if (tm) {
     FFPP_CUDA(h, cudaEventRecord(h->ev[6], st));
@@ -311,6 +321,11 @@ int ffpp_create(const ffpp_params* p, ffpp_handle** out) {
     double Z = 0.0, s2 = 2.0 * (double)p->sigma_cells * (double)p->sigma_cells;
     for (int k = -R; k <= R; ++k) Z += std::exp(-(double)(k * k) / s2);
     for (int k = -R; k <= R; ++k) c.taps[k + R] = (float)(std::exp(-(double)(k * k) / s2) / Z);
+    static const int buckets[] = {FFPP_K5_RADII(FFPP_K5_LIST) 0};
+    int RT = kMaxRadius;
+    for (int i = 0; buckets[i]; ++i) if (buckets[i] >= R && buckets[i] < RT) RT = buckets[i];
+    c.radius_t = RT;
+    for (int k = -R; k <= R; ++k) c.taps_pad[k + RT] = c.taps[k + R];
   }
 
   auto bail = [&](int code, const std::string& msg) { ffpp_destroy(h); return fail(nullptr, code, msg); };
@@ -365,9 +380,15 @@ int ffpp_create(const ffpp_params* p, ffpp_handle** out) {
   else rc = set_kernel_attrs<false, uint64_t>(h);
   if (rc != FFPP_OK) { std::string m = h->err; return bail(rc, m); }
   {
-    const size_t s5 = k5_smem_bytes(R);
-    if ((e = cudaFuncSetAttribute(k5_density, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s5)) != cudaSuccess)
-      return bail(FFPP_ECUDA, std::string("cudaFuncSetAttribute(k5): ") + cudaGetErrorString(e));
+    const size_t s5 = k5_smem_bytes(p->max_frame_w / p->cell_px, c.radius_t);
+    e = cudaSuccess;
+    switch (c.radius_t) {
+#define FFPP_K5_CASE(RT) case RT: e = cudaFuncSetAttribute(k5_density<RT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s5); break;
+      FFPP_K5_RADII(FFPP_K5_CASE)
+#undef FFPP_K5_CASE
+      default: break;
+    }
+    if (e != cudaSuccess) return bail(FFPP_ECUDA, std::string("cudaFuncSetAttribute(k5): ") + cudaGetErrorString(e));
   }
   *out = h;
   return FFPP_OK;

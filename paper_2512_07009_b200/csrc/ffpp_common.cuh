@@ -45,6 +45,8 @@ struct Consts {
   int32_t cell_px;
   int32_t radius;
   float taps[2 * kMaxRadius + 1];
+  int32_t radius_t;                 // compile-time radius bucket RT >= radius that a6 runs with
+  float taps_pad[2 * kMaxRadius + 1];   // taps centred in a 2 RT + 1 window, zero outside the real radius
 };
 
 // ---- development aid: per-phase %globaltimer stamps (compiled only with -DFFPP_PROFILE_PHASES) ----

@@ -965,97 +965,111 @@ __global__ void __launch_bounds__(K4_THREADS, 2) k4_resolve_emit(
 // =====================================================================================================
 // a6 — density convolution (north_star (d); the paper's grid-cell x bird loop,
 // PAPER.md:L203-208, restated as histogram + separable convolution).
-// One CTA per 64 x 32-cell output tile.  The tile's halo'd histogram is read through the reflect fold
-// (fold(i,n) = -i-1 | 2n-1-i, the half-sample symmetric extension) into shared memory as floats, convolved with the
-// normalised taps along x into a second shared buffer and along y into the output, both passes register-blocked
-// (8 outputs per thread slide over an 8-wide window, one shared load per tap).  HBM traffic: 2 bytes per cell of
-// histogram (L2-resident: written by a2/a4 microseconds earlier) + one coalesced 4-byte store per cell.
+// One CTA per strip of K5_TH output rows x up to K5_TW columns of one frame.  The y pass runs FIRST, straight from
+// the uint16 histogram in global memory (L2-resident: a2/a4 wrote it microseconds earlier): a thread owns one
+// column and eight consecutive output rows, reads the 8 + 2R histogram rows it needs through the reflect fold
+// (fold(i,n) = -i-1 | 2n-1-i, the half-sample symmetric extension), and keeps the eight sums in registers; the
+// result goes to shared memory for the strip's columns plus R folded halo columns per side.  The x pass then reads
+// 8 + 2R consecutive floats of one row (float4 loads, row pitch = 4 mod 32 so a quarter warp of eight rows is
+// conflict-free), produces eight consecutive outputs and writes them as one 32-byte sector.  Because the y pass
+// comes first, nothing is computed for halo ROWS: the work is exactly 2(2R+1) FMAs per cell plus 2R/TW for the
+// halo columns.  The tap loops are fully unrolled for the compile-time radius RT >= R (taps zero-padded to RT), so
+// there is no window shifting and every tap is a constant-bank operand.
+// HBM traffic: 2 bytes per cell of histogram (mostly L2 hits) + one 4-byte store per cell.
 // =====================================================================================================
 constexpr int K5_THREADS = 256;
-constexpr int K5_TW = 64, K5_TH = 32;
+constexpr int K5_TH = 16;                       // output rows per CTA (two 8-row register blocks)
+constexpr int K5_TW = 512;                      // output columns per CTA at most (wider grids are tiled in x)
 
-__host__ __device__ inline int k5_hs_stride(int R) { return (K5_TW + 2 * R) | 1; }          // odd: conflict-free column walks
-__host__ __device__ inline size_t k5_smem_bytes(int R) {
-  return sizeof(float) * ((size_t)(K5_TH + 2 * R) * k5_hs_stride(R) + 8 + (size_t)(K5_TH + 2 * R) * (K5_TW + 1));
+__host__ __device__ inline int k5_tile_w(int gw) { return gw < K5_TW ? ((gw + 7) & ~7) : K5_TW; }      // multiple of 8
+__host__ __device__ inline int k5_pitch(int tw, int RT) {                 // >= tw + 2 RT + 2, = 4 mod 32
+  const int need = tw + 2 * RT + 2;
+  return ((need - 4 + 31) / 32) * 32 + 4;
+}
+__host__ __device__ inline size_t k5_smem_bytes(int gw_max, int RT) {
+  return sizeof(float) * (size_t)K5_TH * k5_pitch(k5_tile_w(gw_max), RT);
+}
+__host__ __device__ inline int k5_tiles(int gw, int gh) {
+  const int tw = k5_tile_w(gw);
+  return ((gw + tw - 1) / tw) * ((gh + K5_TH - 1) / K5_TH);
 }
 
+__device__ __forceinline__ int k5_fold(int i, const int n) {
+  i = i < 0 ? -i - 1 : (i >= n ? 2 * n - 1 - i : i);
+  return min(max(i, 0), n - 1);                  // beyond one fold only zero-padded taps look: any in-range cell will do
+}
+
+template <int RT>
 __global__ void __launch_bounds__(K5_THREADS) k5_density(const FrameDesc* __restrict__ frames, Consts cst,
                                                          const uint16_t* __restrict__ hist16,
                                                          float* __restrict__ out_density) {
-  extern __shared__ __align__(16) float smem5[];
+  extern __shared__ __align__(16) float s_t[];              // [K5_TH][P]: y-pass result, column c <-> gx = x0 - RT + c
   const int f = blockIdx.y;
   const FrameDesc* fd = &frames[f];
   const int gw = fd->gw, gh = fd->gh;
-  const int tiles_x = (gw + K5_TW - 1) / K5_TW, tiles_y = (gh + K5_TH - 1) / K5_TH;
+  const int tw = k5_tile_w(gw);
+  const int tiles_x = (gw + tw - 1) / tw, tiles_y = (gh + K5_TH - 1) / K5_TH;
   if ((int)blockIdx.x >= tiles_x * tiles_y) return;
   const int ty = blockIdx.x / tiles_x, tx = blockIdx.x - ty * tiles_x;
-  const int R = cst.radius;
-  const int HW = K5_TW + 2 * R, HH = K5_TH + 2 * R, HS = k5_hs_stride(R), RS = K5_TW + 1;
-  float* hs = smem5;                       // [HH][HS] (+8 floats of slack for the sliding window's last loads)
-  float* rowc = smem5 + (size_t)HH * HS + 8;   // [HH][RS]
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int x0 = tx * tw, y0 = ty * K5_TH;
+  const int P = k5_pitch(tw, RT);
+  const int twh = tw + 2 * RT;
+  const int tid = threadIdx.x;
   const uint16_t* hsrc = hist16 + fd->dens_off;
-  const int ex0 = tx * K5_TW - R, ey0 = ty * K5_TH - R;
+  constexpr int NW = 8 + 2 * RT;                            // window of one 8-output block
 
-  for (int i = tid; i < HH * HW; i += K5_THREADS) {
-    const int ly = i / HW, lx = i - ly * HW;
-    int gy = ey0 + ly, gx = ex0 + lx;
-    gy = gy < 0 ? -gy - 1 : (gy >= gh ? 2 * gh - 1 - gy : gy);
-    gx = gx < 0 ? -gx - 1 : (gx >= gw ? 2 * gw - 1 - gx : gx);
-    float v = 0.0f;
-    if (gy >= 0 && gx >= 0) v = (float)hsrc[(int64_t)gy * gw + gx];   // < 0: overhang beyond the folded range, unused
-    hs[ly * HS + lx] = v;
-  }
-  if (tid < 8) hs[(size_t)HH * HS + tid] = 0.0f;
-  __syncthreads();
-
-  // x pass: rowc[y][x] = sum_k w[k] * hs[y][x + k].  lane -> row, 8 consecutive x per thread.
-  for (int y0 = 0; y0 < HH; y0 += 32) {
-    const int y = y0 + lane;
-    if (y < HH) {
-      const float* hrow = hs + y * HS + warp * 8;
-      float win[8], acc[8];
+  // ---- y pass: unit = (column c, 8-row block q) ----
+  for (int u = tid; u < twh * (K5_TH / 8); u += K5_THREADS) {
+    const int q = u / twh, c = u - q * twh;
+    const int gx = k5_fold(x0 - RT + c, gw);
+    const int yb = y0 + 8 * q - RT;
+    float acc[8];
 #pragma unroll
-      for (int m = 0; m < 8; ++m) { win[m] = hrow[m]; acc[m] = 0.0f; }
-#pragma unroll 8
-      for (int k = 0; k <= 2 * R; ++k) {
-        const float t = cst.taps[k];
+    for (int m = 0; m < 8; ++m) acc[m] = 0.0f;
 #pragma unroll
-        for (int m = 0; m < 8; ++m) acc[m] = fmaf(t, win[m], acc[m]);
-#pragma unroll
-        for (int m = 0; m < 7; ++m) win[m] = win[m + 1];
-        win[7] = hrow[k + 8];
-      }
-#pragma unroll
-      for (int m = 0; m < 8; ++m) rowc[y * RS + warp * 8 + m] = acc[m];
-    }
-  }
-  __syncthreads();
-
-  // y pass + store: thread -> column x, 8 consecutive rows.
-  {
-    const int x = tid & 63, yg = tid >> 6;                 // 4 groups x 8 rows = 32
-    const float* col = rowc + (yg * 8) * RS + x;
-    float win[8], acc[8];
-#pragma unroll
-    for (int m = 0; m < 8; ++m) { win[m] = col[m * RS]; acc[m] = 0.0f; }
-#pragma unroll 8
-    for (int k = 0; k <= 2 * R; ++k) {
-      const float t = cst.taps[k];
-#pragma unroll
-      for (int m = 0; m < 8; ++m) acc[m] = fmaf(t, win[m], acc[m]);
-#pragma unroll
-      for (int m = 0; m < 7; ++m) win[m] = win[m + 1];
-      const int yy = yg * 8 + k + 8;
-      win[7] = yy < HH ? col[(k + 8) * RS] : 0.0f;
-    }
-    const int gx = tx * K5_TW + x;
-    float* out = out_density + fd->dens_off;
-    if (gx < gw) {
+    for (int r = 0; r < NW; ++r) {
+      const float v = (float)hsrc[(int64_t)k5_fold(yb + r, gh) * gw + gx];
 #pragma unroll
       for (int m = 0; m < 8; ++m) {
-        const int gy = ty * K5_TH + yg * 8 + m;
-        if (gy < gh) out[(int64_t)gy * gw + gx] = acc[m];
+        const int k = r - m;                                // compile-time after unrolling
+        if (k >= 0 && k <= 2 * RT) acc[m] = fmaf(cst.taps_pad[k], v, acc[m]);
+      }
+    }
+#pragma unroll
+    for (int m = 0; m < 8; ++m) s_t[(8 * q + m) * P + c] = acc[m];
+  }
+  if (tid < 2 * K5_TH) s_t[(tid >> 1) * P + twh + (tid & 1)] = 0.0f;     // the two slack columns the float4 loads touch
+  __syncthreads();
+
+  // ---- x pass: unit = (row y, 8-column group g); consecutive lanes take consecutive rows ----
+  float* out = out_density + fd->dens_off;
+  const bool vec_ok = ((fd->dens_off | (int64_t)gw) & 3) == 0;
+  for (int u = tid; u < K5_TH * (tw / 8); u += K5_THREADS) {
+    const int g = u / K5_TH, y = u - g * K5_TH;
+    const float4* row4 = reinterpret_cast<const float4*>(s_t + y * P + 8 * g);
+    float win[(NW + 3) & ~3];
+#pragma unroll
+    for (int i = 0; i < (NW + 3) / 4; ++i) {
+      const float4 t = row4[i];
+      win[4 * i] = t.x; win[4 * i + 1] = t.y; win[4 * i + 2] = t.z; win[4 * i + 3] = t.w;
+    }
+    float acc[8];
+#pragma unroll
+    for (int m = 0; m < 8; ++m) {
+      acc[m] = 0.0f;
+#pragma unroll
+      for (int k = 0; k <= 2 * RT; ++k) acc[m] = fmaf(cst.taps_pad[k], win[m + k], acc[m]);
+    }
+    const int gy = y0 + y, gx = x0 + 8 * g;
+    if (gy < gh) {
+      float* dst = out + (int64_t)gy * gw + gx;
+      if (vec_ok && gx + 8 <= gw) {
+        reinterpret_cast<float4*>(dst)[0] = make_float4(acc[0], acc[1], acc[2], acc[3]);
+        reinterpret_cast<float4*>(dst)[1] = make_float4(acc[4], acc[5], acc[6], acc[7]);
+      } else {
+#pragma unroll
+        for (int m = 0; m < 8; ++m)
+          if (gx + m < gw) dst[m] = acc[m];
       }
     }
   }
