@@ -91,6 +91,23 @@ __global__ void __launch_bounds__(K1_THREADS) k1_threshold_compact(const uint8_t
   }
 
   // ---------------- consumer warps ----------------
+  // A slice's survivors are stored one chunk LATER: the atomicAdd that reserves their slots in the frame's list is
+  // issued, the warp releases the ring stage and evaluates the next chunk, and only then reads the returned base,
+  // so the L2 round trip of the (contended, one address per frame) counter is off the critical path.
+  KeyT p_keys[kHalf ? 8 : 4];
+  uint32_t p_pass = 0;
+  int p_total = 0, p_excl = 0, p_base = 0;
+  int64_t p_coff = 0;
+  auto flush_pending = [&]() {
+    if (p_total) {                                              // warp-uniform
+      const int base = __shfl_sync(0xffffffffu, p_base, 31);
+      KeyT* dst = surv_keys + p_coff + base + p_excl;
+#pragma unroll
+      for (int i = 0; i < (kHalf ? 8 : 4); ++i)
+        if ((p_pass >> i) & 1u) *dst++ = p_keys[i];
+      p_total = 0;
+    }
+  };
   int it = 0;
   for (int64_t c = blockIdx.x; c < nchunks; c += gridDim.x, ++it) {
     const int stage = it % K1_STAGES;
@@ -103,7 +120,46 @@ __global__ void __launch_bounds__(K1_THREADS) k1_threshold_compact(const uint8_t
       f0 = lo;
     }
     mbar_wait(&full[stage], (uint32_t)(it / K1_STAGES) & 1u);
-    if (gw0 < total_cand) {
+    if (gw0 + CPW <= total_cand && gw0 + CPW <= coff[f0 + 1]) {
+      // ---- fast path: the warp's whole slice lies in one frame.  A lane owns CPL CONSECUTIVE rows = 80 bytes =
+      // five conflict-free 16-byte shared loads, picks the score word of each row out of registers, and the slice is
+      // compacted in lane order with one shuffle scan and one global atomicAdd ----
+      const uint4* src = reinterpret_cast<const uint4*>(buf + ((size_t)warp * CPW + (size_t)lane * CPL) * ROW);
+      uint32_t w[20];
+#pragma unroll
+      for (int q = 0; q < 5; ++q) { const uint4 t = src[q]; w[4 * q] = t.x; w[4 * q + 1] = t.y; w[4 * q + 2] = t.z; w[4 * q + 3] = t.w; }
+      const int idx0 = (int)(gw0 - coff[f0]) + lane * CPL;
+      KeyT keys[CPL];
+      uint32_t pass = 0;
+#pragma unroll
+      for (int i = 0; i < CPL; ++i) {
+        float z;
+        if (kHalf) {
+          const int hw = 5 * i + 4;
+          const uint16_t h = (uint16_t)(w[hw >> 1] >> (16 * (hw & 1)));
+          z = __half2float(__ushort_as_half(h));
+          if (sizeof(KeyT) == 4) keys[i] = (KeyT)((desc_key16(h) << 16) | (uint32_t)(idx0 + i));
+          else keys[i] = (KeyT)(((uint64_t)desc_key32(z) << 32) | (uint32_t)(idx0 + i));
+        } else {
+          z = __uint_as_float(w[5 * i + 4]);
+          keys[i] = (KeyT)(((uint64_t)desc_key32(z) << 32) | (uint32_t)(idx0 + i));
+        }
+        if (z > T) pass |= 1u << i;
+      }
+      const int c = __popc(pass);
+      int inc = c;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
+      const int total = __shfl_sync(0xffffffffu, inc, 31);
+      flush_pending();                                          // the previous slice: its atomic has had a whole chunk to return
+      if (total) {
+        if (lane == 31) p_base = atomicAdd(&surv_cnt[f0], total);   // not consumed until the next flush
+        p_total = total; p_pass = pass; p_excl = inc - c; p_coff = coff[f0];
+#pragma unroll
+        for (int i = 0; i < CPL; ++i) p_keys[i] = keys[i];
+      }
+    } else if (gw0 < total_cand) {
+      flush_pending();
       KeyT keys[CPL];
       int fr[CPL];
       uint32_t pass = 0;
@@ -144,6 +200,7 @@ __global__ void __launch_bounds__(K1_THREADS) k1_threshold_compact(const uint8_t
     __syncwarp();
     if (lane == 0) mbar_arrive(&empty[stage]);
   }
+  flush_pending();
 }
 
 // =====================================================================================================
@@ -1026,13 +1083,27 @@ __global__ void __launch_bounds__(K5_THREADS) k5_density(const FrameDesc* __rest
     float acc[8];
 #pragma unroll
     for (int m = 0; m < 8; ++m) acc[m] = 0.0f;
+    const uint16_t* col = hsrc + gx;
+    if (yb >= 0 && yb + NW <= gh) {                         // interior block: rows yb .. yb + NW - 1, no fold
+      const uint16_t* pr = col + yb * gw;
 #pragma unroll
-    for (int r = 0; r < NW; ++r) {
-      const float v = (float)hsrc[(int64_t)k5_fold(yb + r, gh) * gw + gx];
+      for (int r = 0; r < NW; ++r) {
+        const float v = (float)pr[r * gw];
 #pragma unroll
-      for (int m = 0; m < 8; ++m) {
-        const int k = r - m;                                // compile-time after unrolling
-        if (k >= 0 && k <= 2 * RT) acc[m] = fmaf(cst.taps_pad[k], v, acc[m]);
+        for (int m = 0; m < 8; ++m) {
+          const int k = r - m;                              // compile-time after unrolling
+          if (k >= 0 && k <= 2 * RT) acc[m] = fmaf(cst.taps_pad[k], v, acc[m]);
+        }
+      }
+    } else {
+#pragma unroll
+      for (int r = 0; r < NW; ++r) {
+        const float v = (float)col[k5_fold(yb + r, gh) * gw];
+#pragma unroll
+        for (int m = 0; m < 8; ++m) {
+          const int k = r - m;
+          if (k >= 0 && k <= 2 * RT) acc[m] = fmaf(cst.taps_pad[k], v, acc[m]);
+        }
       }
     }
 #pragma unroll
