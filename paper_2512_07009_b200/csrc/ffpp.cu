@@ -21,15 +21,17 @@ namespace {
 thread_local std::string g_create_error;
 
 struct DeviceMeta {           // one pinned block + one device block, uploaded with a single copy
-  size_t frames_off, cand_off_off, bytes;
+  size_t frames_off, cand_off_off, block_frame_off, bytes;
 };
 
-DeviceMeta meta_layout(int max_frames) {
+DeviceMeta meta_layout(int max_frames, int64_t max_total_candidates) {
   DeviceMeta m;
   size_t o = 0;
   m.frames_off = o; o += sizeof(FrameDesc) * (size_t)max_frames;
   o = (o + 15) & ~(size_t)15;
   m.cand_off_off = o; o += sizeof(int64_t) * ((size_t)max_frames + 1);
+  o = (o + 15) & ~(size_t)15;
+  m.block_frame_off = o; o += sizeof(int32_t) * ((size_t)(max_total_candidates / K1_BLOCK) + 2);
   m.bytes = (o + 15) & ~(size_t)15;
   return m;
 }
@@ -170,6 +172,15 @@ int schedule(ffpp_handle* h, int B, const int32_t* N, const int32_t* dims, cudaS
   }
   coff[B] = cand;
   if (cand > p.max_total_candidates) return fail(h, FFPP_ECAPACITY, "sum N_f exceeds max_total_candidates");
+  {
+    // a1: first frame of every K1_BLOCK-row block of the flat candidate stream
+    int32_t* bf = reinterpret_cast<int32_t*>(h->h_meta + h->ml.block_frame_off);
+    int f = 0;
+    for (int64_t b = 0; b * K1_BLOCK < cand; ++b) {
+      while (f + 1 < B && coff[f + 1] <= b * K1_BLOCK) ++f;
+      bf[b] = f;
+    }
+  }
   if (cells > h->max_total_cells) return fail(h, FFPP_ECAPACITY, "density cells exceed max_total_cells");
   if (edges > h->edge_cap_total) return fail(h, FFPP_ECAPACITY, "suppression-edge pool exceeds nms_workspace_bytes");
   FFPP_CUDA(h, cudaMemcpyAsync(h->d_meta, h->h_meta, h->ml.bytes, cudaMemcpyHostToDevice, stream));
@@ -198,8 +209,8 @@ int launch_all(ffpp_handle* h, const void* raw, int B, cudaStream_t st, ffpp_box
     int64_t grid = (int64_t)h->sm_count * K1_CTAS_PER_SM;
     if (grid > nchunks) grid = nchunks;
     k1_threshold_compact<kHalf, KeyT><<<(unsigned)grid, K1_THREADS, K1_STAGES * K1_CHUNK_BYTES, st>>>(
-        static_cast<const uint8_t*>(raw), h->total_cand, B, coff, c.logit_thr, static_cast<KeyT*>(h->d_surv_keys),
-        h->surv_cnt());
+        static_cast<const uint8_t*>(raw), h->total_cand, B, coff, reinterpret_cast<const int32_t*>(h->d_meta + h->ml.block_frame_off),
+        c.logit_thr, static_cast<KeyT*>(h->d_surv_keys), h->surv_cnt());
   }
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[2], st));
   // a2 (+ clears the a5 histogram)
@@ -347,7 +358,7 @@ int ffpp_create(const ffpp_params* p, ffpp_handle** out) {
   h->p.nms_edges_per_box = (int32_t)std::min<int64_t>(h->edges_per_box, 0x7fffffff);
   h->edge_cap_total = h->edges_per_box * nmax_cap * p->max_frames;
 
-  h->ml = meta_layout(p->max_frames);
+  h->ml = meta_layout(p->max_frames, p->max_total_candidates);
   auto dalloc = [&](void** ptr, size_t bytes) {
     if (bytes == 0) bytes = 16;
     cudaError_t ee = cudaMalloc(ptr, bytes);

@@ -23,6 +23,7 @@ constexpr int K1_THREADS = 32 * (K1_CONSUMERS + 1);
 constexpr int K1_CHUNK_BYTES = 20480;   // multiple of lcm(16, 10, 20) = 80 and of 8 warps x 32 lanes rows
 constexpr int K1_STAGES = 3;
 constexpr int K1_CTAS_PER_SM = 3;        // 60 KB ring + 8 KB offsets per CTA
+constexpr int K1_BLOCK = 2048;          // rows per entry of the host-built block -> first frame table
 constexpr int K1_SMEM_FRAMES = 1024;    // frame offsets cached in shared memory (larger batches read them from L2)
 
 template <bool kHalf, typename KeyT>
@@ -42,7 +43,8 @@ __device__ __forceinline__ bool k1_eval(const uint8_t* buf, int gl, float T, int
 
 template <bool kHalf, typename KeyT>
 __global__ void __launch_bounds__(K1_THREADS) k1_threshold_compact(const uint8_t* __restrict__ raw, int64_t total_cand,
-                                                                   int B, const int64_t* __restrict__ cand_off, float T,
+                                                                   int B, const int64_t* __restrict__ cand_off,
+                                                                   const int32_t* __restrict__ block_frame, float T,
                                                                    KeyT* __restrict__ surv_keys,
                                                                    int* __restrict__ surv_cnt) {
   constexpr int ROW = kHalf ? 10 : 20;
@@ -114,10 +116,9 @@ __global__ void __launch_bounds__(K1_THREADS) k1_threshold_compact(const uint8_t
     const uint8_t* buf = ring + (size_t)stage * K1_CHUNK_BYTES;
     const int64_t gw0 = c * CPC + (int64_t)warp * CPW;          // first candidate of this warp's slice
     int f0 = 0;
-    if (gw0 < total_cand) {                                     // frame of gw0 (overlaps the copy)
-      int lo = 0, hi = B;
-      while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (coff[mid] <= gw0) lo = mid; else hi = mid; }
-      f0 = lo;
+    if (gw0 < total_cand) {                                     // frame of gw0 (overlaps the copy): table + short walk
+      f0 = block_frame[gw0 / K1_BLOCK];
+      while (coff[f0 + 1] <= gw0) ++f0;
     }
     mbar_wait(&full[stage], (uint32_t)(it / K1_STAGES) & 1u);
     if (gw0 + CPW <= total_cand && gw0 + CPW <= coff[f0 + 1]) {
