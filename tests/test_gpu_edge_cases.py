@@ -139,6 +139,53 @@ def test_max_topk_for_both_key_widths(env):
     check(env, w32)
 
 
+def test_keep_everything_at_max_topk_takes_the_global_sort_scratch(env):
+    """thr >= 1 keeps the whole top-K list, so the kept set (24576 / 12288 boxes) is far beyond what a4 can order in
+    shared memory: the radix passes run on the global scratch arrays."""
+    rng = np.random.default_rng(9)
+    N = 42840
+    raw = frame(N, np.float16, rng, 0)
+    raw[:, 4] = rng.uniform(-1.0, 8.0, size=N)
+    raw[:, :4] = rng.uniform(0.1, 0.6, size=(N, 4))
+    w = W(raw, [[1920, 1088]], dict(P, top_k=24576, iou_thresh=1.0, sigma_cells=2.0))
+    out, ref = check(env, w)
+    assert ref.counts[0] == 24576
+    w32 = W(raw.astype(np.float32), [[1920, 1088]], dict(P, dtype="fp32", top_k=12288, iou_thresh=1.0, sigma_cells=2.0))
+    out, ref = check(env, w32)
+    assert ref.counts[0] == 12288
+
+
+@pytest.mark.parametrize("thr", [0.0, 0.02, 0.05, 0.3, 0.5, 0.7, 0.95])
+def test_wild_box_sizes_against_every_threshold(env, thr):
+    """Boxes from a fraction of a pixel to several frames wide, nested and far outside the frame: the a3 partner window
+    (rho * own size around the own centre, in spatial cells) must still reach every pair the oracle's all-pairs walk sees."""
+    rng = np.random.default_rng(int(thr * 100) + 11)
+    N = 8400
+    raw = frame(N, np.float32, rng, 0)
+    js = rng.choice(N, size=3000, replace=False)
+    raw[js, :4] = np.exp(rng.uniform(np.log(0.02), np.log(60.0), size=(3000, 4))).astype(np.float32)
+    big = js[:40]
+    raw[big, :4] = rng.uniform(30.0, 120.0, size=(40, 4))            # boxes that cover the whole frame and more
+    twins = js[100:400]
+    raw[twins, :4] = raw[twins[0], :4] * rng.uniform(0.97, 1.03, size=(300, 4))   # a pile of near-identical shapes
+    raw[js, 4] = rng.uniform(-1.0, 8.0, size=3000)
+    w = W(raw, [[640, 640]], dict(P, dtype="fp32", top_k=2500, iou_thresh=thr))
+    check(env, w, nms_edges_per_box=1300)               # room for every pair: at thr ~ 0 the frame-sized boxes touch everything
+
+
+@pytest.mark.parametrize("sigma,trunc,R", [(0.5, 3.0, 1), (1.0, 3.0, 3), (1.7, 3.0, 5), (3.7, 3.0, 11), (4.4, 3.0, 13),
+                                            (5.8, 3.0, 17), (7.0, 3.0, 21), (10.0, 3.0, 30), (8.0, 4.0, 32)])
+def test_every_radius_bucket_of_the_density_kernel(env, sigma, trunc, R):
+    """a6 is compiled for a list of radii and runs the smallest one >= R with zero-padded taps."""
+    rng = np.random.default_rng(12)
+    dims = [[640, 640], [1280, 720], [320, 320]]
+    parts = [frame(env[3].frame_candidates(a, b), np.float16, rng, 300, lo=0.0, hi=8.0) for a, b in dims]
+    w = W(np.concatenate(parts), dims, dict(P, sigma_cells=sigma, truncate_sigmas=trunc, iou_thresh=0.5))
+    torch, m, oracle_mod, _ = env
+    assert oracle_mod.taps(sigma, trunc)[0] == R
+    check(env, w)
+
+
 def test_abi_misuse_is_rejected(env):
     torch, m, oracle_mod, gen = env
     good = dict(max_frames=2, max_total_candidates=2 * 8400, max_frame_w=640, max_frame_h=640)
