@@ -449,16 +449,32 @@ int ffpp_run_host(ffpp_handle* h, const void* raw, int32_t B, const int32_t* N_p
   FFPP_CUDA(h, cudaMemcpyAsync(h->d_in, raw, (size_t)cand * 5 * esz, cudaMemcpyHostToDevice, st));
   int rc = ffpp_run(h, h->d_in, B, N_per_frame, frame_dims, stream, h->d_out_boxes, h->d_out_counts, h->d_out_density);
   if (rc != FFPP_OK) return rc;
+  // kept boxes: only rows [0, count) of each frame are defined.  A pinned (device-mapped) out_boxes is written by one
+  // kernel through its device alias; a pageable one gets one copy per frame after the counts have arrived.
+  const size_t K = (size_t)h->p.top_k;
+  ffpp_box* alias = nullptr;
+  {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, out_boxes) == cudaSuccess && at.type == cudaMemoryTypeHost && at.devicePointer)
+      alias = static_cast<ffpp_box*>(at.devicePointer);
+    else
+      cudaGetLastError();
+  }
+  if (alias) {
+    const dim3 g((unsigned)std::min<size_t>(16, (K * 3 + KH_THREADS - 1) / KH_THREADS), (unsigned)B);
+    kh_copy_kept_rows<<<g, KH_THREADS, 0, st>>>(h->d_out_boxes, h->d_out_counts, (int)K, alias);
+  }
   FFPP_CUDA(h, cudaMemcpyAsync(out_counts, h->d_out_counts, sizeof(int) * (size_t)B, cudaMemcpyDeviceToHost, st));
   FFPP_CUDA(h, cudaMemcpyAsync(out_density, h->d_out_density, sizeof(float) * (size_t)cells, cudaMemcpyDeviceToHost, st));
   FFPP_CUDA(h, cudaStreamSynchronize(st));
-  // only rows [0, count) of each frame are defined: copy exactly those
-  const size_t K = (size_t)h->p.top_k;
-  for (int f = 0; f < B; ++f)
-    if (out_counts[f] > 0)
-      FFPP_CUDA(h, cudaMemcpyAsync(out_boxes + (size_t)f * K, h->d_out_boxes + (size_t)f * K, sizeof(ffpp_box) * (size_t)out_counts[f],
-                                   cudaMemcpyDeviceToHost, st));
-  FFPP_CUDA(h, cudaStreamSynchronize(st));
+  if (!alias) {
+    for (int f = 0; f < B; ++f)
+      if (out_counts[f] > 0)
+        FFPP_CUDA(h, cudaMemcpyAsync(out_boxes + (size_t)f * K, h->d_out_boxes + (size_t)f * K, sizeof(ffpp_box) * (size_t)out_counts[f],
+                                     cudaMemcpyDeviceToHost, st));
+    FFPP_CUDA(h, cudaStreamSynchronize(st));
+  }
+  FFPP_CUDA(h, cudaGetLastError());
   return FFPP_OK;
 }
 

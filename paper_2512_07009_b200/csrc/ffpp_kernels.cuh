@@ -1147,4 +1147,20 @@ __global__ void __launch_bounds__(K5_THREADS) k5_density(const FrameDesc* __rest
   }
 }
 
+// =====================================================================================================
+// Host-buffer path only (ffpp_run_host): copy rows [0, count) of every frame's kept list from the device staging
+// buffer straight into the caller's PINNED host array through its device alias (zero-copy stores over PCIe): one
+// launch instead of one cudaMemcpyAsync per frame.
+// =====================================================================================================
+constexpr int KH_THREADS = 256;
+__global__ void __launch_bounds__(KH_THREADS) kh_copy_kept_rows(const ffpp_box* __restrict__ src, const int* __restrict__ counts,
+                                                                int K, ffpp_box* __restrict__ dst_host_alias) {
+  const int f = blockIdx.y;
+  const int n = counts[f];
+  const int64_t base = (int64_t)f * K * 3;                     // in 8-byte words: a record is three of them
+  const uint2* s = reinterpret_cast<const uint2*>(src) + base;
+  uint2* d = reinterpret_cast<uint2*>(dst_host_alias) + base;
+  for (int i = blockIdx.x * KH_THREADS + threadIdx.x; i < n * 3; i += gridDim.x * KH_THREADS) d[i] = s[i];
+}
+
 }  // namespace ffpp

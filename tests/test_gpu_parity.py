@@ -109,6 +109,23 @@ def test_host_buffer_entry_point(torch_cuda, ffpp_mod, oracle_mod, gen_mod):
     compare(out, oracle_mod.run(w.params, w.raw, w.N_per_frame, w.frame_dims), w)
 
 
+def test_host_buffer_entry_point_with_pinned_buffers(torch_cuda, ffpp_mod, oracle_mod, gen_mod):
+    """Pinned (device-mapped) host outputs: the kept rows are written by one kernel through the device alias of
+    out_boxes instead of one copy per frame; the result is the same."""
+    torch = torch_cuda
+    w = gen_mod.make_config(5, B=8)
+    pp = ffpp_mod.FFPP.for_workload(w)
+    out = ffpp_mod.Output()
+    out.density_offsets = pp.density_offsets(w.frame_dims)
+    out.boxes = torch.zeros((w.B, pp.top_k, 6), dtype=torch.float32).pin_memory()
+    out.counts = torch.zeros((w.B,), dtype=torch.int32).pin_memory()
+    out.density = torch.zeros((int(out.density_offsets[-1]),), dtype=torch.float32).pin_memory()
+    raw = torch.from_numpy(w.raw).pin_memory()
+    for _ in range(2):
+        pp.run_host(raw, w.N_per_frame, w.frame_dims, out=out)
+    compare(out, oracle_mod.run(w.params, w.raw, w.N_per_frame, w.frame_dims), w)
+
+
 @pytest.mark.parametrize("c", [3, 4, 5])
 def test_full_size_configs_in_the_bench_launch_configuration(torch_cuda, ffpp_mod, oracle_mod, gen_mod, c):
     """BASELINE.json's full sizes (configs 3-5: 32 / 64 / 256 frames), same handle sizing and launch
