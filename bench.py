@@ -239,6 +239,16 @@ def run_ours(args):
     pp.set_stage_timing(False)
     stage_ms = np.mean(np.stack(stage), axis=0)
 
+    # ---- calibration: a plain read of the same raw buffer, same cold-L2 regime, CUDA events on the same stream ----
+    rd = []
+    for _ in range(8):
+        flush.zero_()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream); pp.stream_read(raw_dev, stream); e1.record(stream)
+        torch.cuda.synchronize()
+        rd.append(e0.elapsed_time(e1))
+    read_floor_ms = float(np.median(rd[2:]))
+
     # ---- e2e: host buffers through ffpp_run_host ----
     cells = int(out.density_offsets[-1])
     h_boxes = torch.empty((B, pp.top_k, 6), dtype=torch.float32).pin_memory()
@@ -300,6 +310,12 @@ def run_ours(args):
             if nm in alg_bytes:
                 gbs = alg_bytes[nm] / (stage_ms[i] * 1e-3) / 1e9
                 stages[nm].update({"algorithmic_bytes": alg_bytes[nm], "GB/s": gbs, "frac_of_hbm_peak": gbs / hbm_peak})
+        s1 = stages["a1_threshold_compact"]
+        s1["plain_read_of_same_bytes"] = {"ms": read_floor_ms, "GB/s": total_cand * row_b / (read_floor_ms * 1e-3) / 1e9,
+                                          "frac_of_hbm_peak": total_cand * row_b / (read_floor_ms * 1e-3) / 1e9 / hbm_peak,
+                                          "note": "k0_stream_read over the raw head output, cold L2 after the same 512 MB write "
+                                                  "flush: what a pure read of this many bytes reaches on this GPU"}
+        s1["frac_of_plain_read"] = read_floor_ms / float(stage_ms[1])
         s3 = stages["a3_nms_mask"]; s3["iou_pairs"] = pairs
         s3["Gpairs/s"] = pairs / (stage_ms[3] * 1e-3) / 1e9
         # a3 ALU ceiling of the all-pairs method: 148 SM x 128 fp32 lanes x clock / 15 instr per IoU pair
@@ -323,9 +339,20 @@ def run_ours(args):
         roofline["avg_launch_ms"] = float(stage_ms[dom])
         roofline["hbm_peak_source"] = peak_src
         tr_path = os.path.join(ROOT, "profiles", f"traffic_config{c}.json")
-        if os.path.exists(tr_path):      # dram bytes per launch from the committed ncu --set full capture
+        if os.path.exists(tr_path):      # per-launch numbers of the committed ncu --set full capture of this config
             with open(tr_path) as fh:
-                roofline["traffic"] = json.load(fh).get(roofline["kernel"])
+                tr = json.load(fh)
+            k = tr.get("kernels", {}).get(roofline["kernel"])
+            if k:
+                roofline["traffic"] = k["dram_bytes"]            # dram__bytes_read.sum + dram__bytes_write.sum
+                roofline["traffic_source"] = tr.get("source")
+                # issue-slot view of the same launch: warp instructions of the capture over the LIVE duration,
+                # against 4 schedulers x 1 warp instruction per clock per SM
+                issue_peak = 148 * 4 * sm_max_mhz * 1e6
+                roofline["issue"] = {"warp_instructions": k["warp_instructions"],
+                                     "achieved_Ginst_s": k["warp_instructions"] / (float(stage_ms[dom]) * 1e-3) / 1e9,
+                                     "peak_Ginst_s": issue_peak / 1e9,
+                                     "frac": k["warp_instructions"] / (float(stage_ms[dom]) * 1e-3) / issue_peak}
         # whole step against HBM: bytes the path must move (raw in, three outputs out) / device step time
         step_bytes = total_cand * row_b + 24 * kept_n + 4 * B + cell_b
         step_gbs = step_bytes / (float(np.median(step_ms)) * 1e-3) / 1e9

@@ -54,8 +54,8 @@ typedef struct ffpp_params {
   int64_t max_total_cells; /* capacity: sum_f (W_f/cell)(H_f/cell); 0 = max_frames * (max_w/cell)(max_h/cell)       */
   int64_t nms_workspace_bytes; /* capacity of the NMS suppression-edge pool in bytes (4 per edge, shared out to the
                                   frames in proportion to min(N_f, top_k)); 0 = nms_edges_per_box edges per box       */
-  int32_t nms_edges_per_box; /* 0 = 16.  An edge is one pair (a, b) with IoU > iou_thresh, b before a in the order; the
-                                flock workloads have 4-8 per box.  A frame that needs more than its share reports
+  int32_t nms_edges_per_box; /* 0 = 16.  An edge is one unordered pair {a, b} with IoU > iou_thresh; the flock
+                                workloads have 4-9 per box.  A frame that needs more than its share reports
                                 out_counts[f] = -1 and leaves its out_boxes / out_density rows undefined              */
   int32_t reserved_;
 } ffpp_params;
@@ -135,6 +135,11 @@ int ffpp_get_stage_ms(ffpp_handle* h, float* ms_out /*HOST [FFPP_NUM_STAGES]*/);
  *   what = 3: decoded boxes of the top-K set, same order        dst HOST float [B][top_k][4]
  * Not part of the contract of the path; used to localise a parity failure. */
 int ffpp_debug_read(ffpp_handle* h, int32_t what, void* dst /*HOST*/, int64_t dst_bytes);
+
+/* Calibration only: enqueue a plain coalesced read of `bytes` bytes of the DEVICE buffer `dev` (16-byte aligned) on
+ * `stream`.  Computes nothing of the path; bench.py times it over the raw head output, under the same cold-cache
+ * regime as stage a1, to report what a pure read of that size achieves on this GPU. */
+int ffpp_debug_stream_read(ffpp_handle* h, const void* dev /*DEVICE*/, int64_t bytes, void* stream);
 
 #ifdef __cplusplus
 }

@@ -43,7 +43,7 @@ NMS_ALU_OPS_PER_PAIR = 15
 BOX_DTYPE = np.dtype([("x1", "<f4"), ("y1", "<f4"), ("x2", "<f4"), ("y2", "<f4"), ("score", "<f4"), ("cand_index", "<i4")])
 
 EXPORTS = ["ffpp_create", "ffpp_run", "ffpp_run_host", "ffpp_destroy", "ffpp_last_error", "ffpp_get_info",
-           "ffpp_set_stage_timing", "ffpp_get_stage_ms", "ffpp_debug_read"]
+           "ffpp_set_stage_timing", "ffpp_get_stage_ms", "ffpp_debug_read", "ffpp_debug_stream_read"]
 
 
 class FFPPParams(ctypes.Structure):
@@ -109,6 +109,8 @@ def load_library() -> ctypes.CDLL:
         L.ffpp_get_stage_ms.argtypes = [vp, vp]
         L.ffpp_debug_read.restype = ctypes.c_int
         L.ffpp_debug_read.argtypes = [vp, i32, vp, i64]
+        L.ffpp_debug_stream_read.restype = ctypes.c_int
+        L.ffpp_debug_stream_read.argtypes = [vp, vp, i64, vp]
         _lib = L
     return _lib
 
@@ -274,6 +276,12 @@ class FFPP:
         ms = np.zeros(NUM_STAGES, dtype=np.float32)
         self._check(self._lib.ffpp_get_stage_ms(self._h, ms.ctypes.data))
         return ms
+
+    def stream_read(self, dev_tensor, stream=None):
+        """ffpp_debug_stream_read: enqueue a plain read of a device tensor (calibration of the a1 roofline)."""
+        st = stream if stream is not None else self._torch.cuda.current_stream()
+        self._check(self._lib.ffpp_debug_stream_read(self._h, dev_tensor.data_ptr(), dev_tensor.numel() * dev_tensor.element_size(),
+                                                     st.cuda_stream))
 
     def debug_read(self, what: int, B: int) -> np.ndarray:
         K = self.top_k

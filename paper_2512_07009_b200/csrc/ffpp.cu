@@ -567,6 +567,18 @@ int ffpp_debug_read(ffpp_handle* h, int32_t what, void* dst, int64_t dst_bytes) 
 
 }
 
+int ffpp_debug_stream_read(ffpp_handle* h, const void* dev, int64_t bytes, void* stream) {
+  if (!h || !dev || bytes < 0) return FFPP_EINVAL;
+  if (reinterpret_cast<uintptr_t>(dev) & 15) return fail(h, FFPP_EINVAL, "buffer must be 16-byte aligned");
+  const int64_t n16 = bytes / 16;
+  if (n16 == 0) return FFPP_OK;
+  const int64_t grid = std::min<int64_t>((int64_t)h->sm_count * 8, (n16 + 255) / 256);
+  k0_stream_read<<<(unsigned)grid, 256, 0, static_cast<cudaStream_t>(stream)>>>(static_cast<const uint4*>(dev), n16,
+                                                                               reinterpret_cast<uint32_t*>(h->d_counters));
+  FFPP_CUDA(h, cudaGetLastError());
+  return FFPP_OK;
+}
+
 #ifdef FFPP_PROFILE_PHASES
 // development aid, compiled only with -DFFPP_PROFILE_PHASES: %globaltimer stamps of the a4 phases of the last run
 int ffpp_debug_phases(unsigned long long* dst, int frames) {

@@ -34,8 +34,10 @@ def test_binary_is_sm100a_and_uses_the_bulk_copy_engine():
     path = m.build()
     elf = subprocess.run(["cuobjdump", "-lelf", path], capture_output=True, text=True).stdout
     assert "sm_100a" in elf, elf
-    sass = subprocess.run(["cuobjdump", "-sass", "-fun", "_ZN4ffpp20k1_threshold_compactILb1EjEEvPKhliPKlfPT0_Pi", path],
-                          capture_output=True, text=True).stdout
+    syms = subprocess.run(["cuobjdump", "-elf", path], capture_output=True, text=True).stdout
+    k1 = sorted(set(re.findall(r"(_ZN4ffpp20k1_threshold_compactILb1EjEE\w+)", syms)))
+    assert k1, "k1_threshold_compact<true, uint32_t> not found in the fatbin"
+    sass = subprocess.run(["cuobjdump", "-sass", "-fun", k1[0], path], capture_output=True, text=True).stdout
     assert "UBLKCP" in sass          # cp.async.bulk (TMA engine) in the HBM-bound streaming kernel
 
 
