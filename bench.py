@@ -167,6 +167,20 @@ def run_reference(args):
     return 0
 
 
+def reduce_over_ranks(total_ms: float, t_e2e: float, frames: float, cands: float, world: int, device):
+    """Whole-job numbers of a weak-scaling run: times are the MAX over ranks, units are the SUM over ranks.
+    No data-path collective exists (frames are independent); these two all-reduces are the only communication."""
+    if world <= 1:
+        return total_ms, t_e2e, frames, cands
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([total_ms, t_e2e], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    u = torch.tensor([frames, cands], dtype=torch.float64, device=device)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t[0]), float(t[1]), float(u[0]), float(u[1])
+
+
 # --------------------------------------------------------------------------------------------------------------
 # our arm
 # --------------------------------------------------------------------------------------------------------------
@@ -276,15 +290,7 @@ def run_ours(args):
     d2h = int(4 * B + 4 * cells + 24 * int(kept.sum()))
 
     # ---- reduce over ranks ----
-    if world > 1:
-        t = torch.tensor([total_ms, t_e2e], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms, t_e2e = float(t[0]), float(t[1])
-        u = torch.tensor([B, total_cand], dtype=torch.float64, device="cuda")
-        dist.all_reduce(u, op=dist.ReduceOp.SUM)
-        frames_all, cand_all = float(u[0]), float(u[1])
-    else:
-        frames_all, cand_all = float(B), float(total_cand)
+    total_ms, t_e2e, frames_all, cand_all = reduce_over_ranks(total_ms, t_e2e, float(B), float(total_cand), world, "cuda")
 
     if rank == 0:
         K = args.steps

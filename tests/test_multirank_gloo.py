@@ -1,0 +1,36 @@
+"""N > 1 host logic on CPU (gloo, world_size 2): bench.py's weak-scaling reduction and the reference arm's
+"rank 0 alone runs and prints" rule.  The data path itself has no collective (frames are independent)."""
+import json
+import os
+import socket
+import subprocess
+import sys
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _free_port() -> int:
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _torchrun(script_args, timeout=300):
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", str(_free_port())] + script_args
+    return subprocess.run(cmd, capture_output=True, text=True, timeout=timeout, cwd=ROOT)
+
+
+def test_weak_scaling_reduction_over_two_gloo_ranks():
+    r = _torchrun([os.path.join(ROOT, "tests", "_gloo_worker.py")])
+    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-4000:]
+    assert "gloo worker ok" in r.stdout
+
+
+def test_reference_arm_under_two_ranks_prints_one_line_from_rank_0():
+    r = _torchrun([os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--config", "1", "--steps", "1", "--warmup", "0"])
+    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-4000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, lines
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["value"] > 0 and d["cpu_baseline"]["kind"] == "oracle"
