@@ -388,13 +388,8 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
         for (int u = 0; u < 4; ++u) { const int i = base + u * K2_THREADS + lane; key[u] = i < n ? gk[i] : ~(KeyT)0; }
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
-          if (base + u * K2_THREADS < n) {                      // warp-uniform
-            const int i = base + u * K2_THREADS + lane;
-            const bool m = i < n && (key[u] & maskbits) == prefix;
-            const uint32_t dg = m ? (uint32_t)((key[u] >> shift) & dmask) : 0xFFFFFFFFu;
-            const uint32_t peers = __match_any_sync(0xffffffffu, dg);
-            if (m && lane == __ffs(peers) - 1) atomicAdd(&cnt[dg], (uint32_t)__popc(peers));
-          }
+          const int i = base + u * K2_THREADS + lane;
+          if (i < n && (key[u] & maskbits) == prefix) atomicAdd(&cnt[(uint32_t)((key[u] >> shift) & dmask)], 1u);
         }
       }
       __syncthreads();
@@ -428,17 +423,26 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
     if (!done) thr = prefix;
   }
 
-  // ---- (2) gather the selected keys into shared memory ----
-  for (int base = warp * 32; base < n; base += K2_THREADS) {
-    const int i = base + lane;
-    KeyT key = 0;
-    bool m = false;
-    if (i < n) { key = gk[i]; m = key <= thr; }
-    const uint32_t bal = __ballot_sync(0xffffffffu, m);
-    int at = 0;
-    if (lane == 0 && bal) at = atomicAdd(&misc->counter, __popc(bal));
-    at = __shfl_sync(0xffffffffu, at, 0);
-    if (m) sel[at + __popc(bal & ((1u << lane) - 1u))] = key;
+  // ---- (2) gather the selected keys into shared memory: count per warp, scan the warps, then place (two sweeps
+  // over the L2-resident keys instead of one shared atomic per warp step on a single hot counter) ----
+  {
+    int mine = 0;
+    for (int base = warp * 32; base < n; base += K2_THREADS) {
+      const int i = base + lane;
+      mine += __popc(__ballot_sync(0xffffffffu, i < n && gk[i] <= thr));
+    }
+    int total;
+    const int inc = blk_scan_inclusive(lane == 0 ? mine : 0, misc, 0, tid, &total);
+    int at = __shfl_sync(0xffffffffu, inc, 0) - mine;            // first slot of this warp
+    for (int base = warp * 32; base < n; base += K2_THREADS) {
+      const int i = base + lane;
+      KeyT key = 0;
+      bool m = false;
+      if (i < n) { key = gk[i]; m = key <= thr; }
+      const uint32_t bal = __ballot_sync(0xffffffffu, m);
+      if (m) sel[at + __popc(bal & ((1u << lane) - 1u))] = key;
+      at += __popc(bal);
+    }
   }
   for (int i = tid; i < K2_CNT_WORDS; i += K2_THREADS) cnt[i] = 0u;
   __syncthreads();
@@ -446,38 +450,51 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
   // ---- (3) decode (O1, O2) + spatial bin ----
   const int64_t obase = (int64_t)f * cst.kpad;
   const float cmx = (float)((fd.cgw << fd.hshift) - 1), cmy = (float)((fd.cgh << fd.hshift) - 1);
-  for (int i = tid; i < nsel; i += K2_THREADS) {
-    const KeyT key = sel[i];
-    const int idx = idx_of_key<KeyT>(key);
-    int l = 0;
-    while (l + 1 < cst.num_levels && idx >= fd.lvl_start[l + 1]) ++l;
-    const int k = idx - fd.lvl_start[l];
-    const int gw = fd.lvl_gw[l];
-    const int iy = k / gw, ix = k - iy * gw;
-    const float s = (float)(1 << cst.stride_log2[l]);
-    float v[4];
-    const int64_t row = fd.cand_off + idx;
-    if (kHalf) {
-      const __half* p = reinterpret_cast<const __half*>(raw) + row * 5;
+  for (int i0 = tid; i0 < nsel; i0 += 4 * K2_THREADS) {
+    float v[4][4];
+    float ps[4][3];                                                // px, py, stride
 #pragma unroll
-      for (int e = 0; e < 4; ++e) v[e] = __half2float(p[e]);
-    } else {
-      const float* p = reinterpret_cast<const float*>(raw) + row * 5;
+    for (int u = 0; u < 4; ++u) {
+      const int i = i0 + u * K2_THREADS;
+      if (i < nsel) {
+        const int idx = idx_of_key<KeyT>(sel[i]);
+        int l = 0;
+        while (l + 1 < cst.num_levels && idx >= fd.lvl_start[l + 1]) ++l;
+        const int k = idx - fd.lvl_start[l];
+        const int gw = fd.lvl_gw[l];
+        const int iy = k / gw, ix = k - iy * gw;
+        const float s = (float)(1 << cst.stride_log2[l]);
+        ps[u][0] = __fmul_rn((float)ix + 0.5f, s); ps[u][1] = __fmul_rn((float)iy + 0.5f, s); ps[u][2] = s;
+        const int64_t row = fd.cand_off + idx;
+        if (kHalf) {
+          const __half* p = reinterpret_cast<const __half*>(raw) + row * 5;
 #pragma unroll
-      for (int e = 0; e < 4; ++e) v[e] = p[e];
+          for (int e = 0; e < 4; ++e) v[u][e] = __half2float(p[e]);
+        } else {
+          const float* p = reinterpret_cast<const float*>(raw) + row * 5;
+#pragma unroll
+          for (int e = 0; e < 4; ++e) v[u][e] = p[e];
+        }
+      }
     }
-    const float px = __fmul_rn((float)ix + 0.5f, s), py = __fmul_rn((float)iy + 0.5f, s);
-    float4 box;
-    box.x = __fsub_rn(px, __fmul_rn(v[0], s));
-    box.y = __fsub_rn(py, __fmul_rn(v[1], s));
-    box.z = __fadd_rn(px, __fmul_rn(v[2], s));
-    box.w = __fadd_rn(py, __fmul_rn(v[3], s));
-    sel_box[obase + i] = box;
-    const uint32_t h = (uint32_t)(cell_coord(box_centre(box.y, box.w), cmy, fd.hshift) * fd.cgw +
-                                  cell_coord(box_centre(box.x, box.z), cmx, fd.hshift));
-    const uint32_t sh = 16u * (h & 1u);
-    const uint32_t old = atomicAdd(&cnt[h >> 1], 1u << sh);
-    aux[i] = (h << 16) | ((old >> sh) & 0xFFFFu);
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int i = i0 + u * K2_THREADS;
+      if (i < nsel) {
+        const float s = ps[u][2];
+        float4 box;
+        box.x = __fsub_rn(ps[u][0], __fmul_rn(v[u][0], s));
+        box.y = __fsub_rn(ps[u][1], __fmul_rn(v[u][1], s));
+        box.z = __fadd_rn(ps[u][0], __fmul_rn(v[u][2], s));
+        box.w = __fadd_rn(ps[u][1], __fmul_rn(v[u][3], s));
+        sel_box[obase + i] = box;
+        const uint32_t h = (uint32_t)(cell_coord(box_centre(box.y, box.w), cmy, fd.hshift) * fd.cgw +
+                                      cell_coord(box_centre(box.x, box.z), cmx, fd.hshift));
+        const uint32_t sh = 16u * (h & 1u);
+        const uint32_t old = atomicAdd(&cnt[h >> 1], 1u << sh);
+        aux[i] = (h << 16) | ((old >> sh) & 0xFFFFu);
+      }
+    }
   }
   __syncthreads();
 
@@ -499,13 +516,21 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
   }
   __syncthreads();
   const uint16_t* base16 = reinterpret_cast<const uint16_t*>(cnt);
-  for (int i = tid; i < nsel; i += K2_THREADS) {
-    const uint32_t a = aux[i];
-    const int pos = (int)base16[a >> 16] + (int)(a & 0xFFFFu);
-    const float4 box = sel_box[obase + i];
-    sp_box[obase + pos] = box;
-    sp_sbox[obase + pos] = shrink_box(box, cst.shrink);
-    sp_key[obase + pos] = sel[i];
+  for (int i0 = tid; i0 < nsel; i0 += 4 * K2_THREADS) {
+    float4 box[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) { const int i = i0 + u * K2_THREADS; if (i < nsel) box[u] = sel_box[obase + i]; }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int i = i0 + u * K2_THREADS;
+      if (i < nsel) {
+        const uint32_t a = aux[i];
+        const int pos = (int)base16[a >> 16] + (int)(a & 0xFFFFu);
+        sp_box[obase + pos] = box[u];
+        sp_sbox[obase + pos] = shrink_box(box[u], cst.shrink);
+        sp_key[obase + pos] = sel[i];
+      }
+    }
   }
   // cell-start table: after the scan the counter words ARE the uint16 start positions in cell order
   {
