@@ -217,7 +217,7 @@ int launch_all(ffpp_handle* h, const void* raw, int B, cudaStream_t st, ffpp_box
   k2_select_bin<kHalf, KeyT><<<B, K2_THREADS, k2_smem_bytes((size_t)c.top_k, sizeof(KeyT)), st>>>(
       static_cast<const uint8_t*>(raw), frames, static_cast<const KeyT*>(h->d_surv_keys), h->surv_cnt(), c,
       h->d_sel_box, h->d_sp_box, h->d_sp_sbox, static_cast<KeyT*>(h->d_sp_key), h->d_cellstart, h->n_sorted(), h->d_hist32,
-      reinterpret_cast<uint32_t*>(h->d_hasin));
+      reinterpret_cast<uint32_t*>(h->d_hasin), h->sm_count);
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[3], st));
   // a3
   {

@@ -333,6 +333,7 @@ __device__ __forceinline__ bool blk_lsd_pass(const T* src, T* dst, int n, int sh
 // =====================================================================================================
 constexpr int K2_THREADS = BLK_THREADS;
 constexpr int K2_SEL_BITS = 12;
+constexpr int K2_MAXPERM = 4096;               // batches up to this many frames get the size-ordered CTA -> frame map
 constexpr int K2_HBINS = kMaxCells;
 constexpr int K2_CNT_WORDS = K2_HBINS / 2;     // 32 KB: 4096 select counters (uint32) or 16384 Hilbert counters (uint16)
 
@@ -345,7 +346,7 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
     const uint8_t* __restrict__ raw, const FrameDesc* __restrict__ frames, const KeyT* __restrict__ surv_keys,
     const int* __restrict__ surv_cnt, Consts cst, float4* __restrict__ sel_box, float4* __restrict__ sp_box,
     float4* __restrict__ sp_sbox, KeyT* __restrict__ sp_key, uint16_t* __restrict__ cellstart,
-    int* __restrict__ n_sorted, uint32_t* __restrict__ hist32, uint32_t* __restrict__ hasin) {
+    int* __restrict__ n_sorted, uint32_t* __restrict__ hist32, uint32_t* __restrict__ hasin, int sm_count) {
   constexpr int KB = sizeof(KeyT) * 8;
   extern __shared__ __align__(16) uint8_t smem[];
   const int K = cst.top_k;
@@ -355,7 +356,28 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
   BlkMisc* misc = reinterpret_cast<BlkMisc*>(cnt + K2_CNT_WORDS);
   __shared__ FrameDesc fd;
 
-  const int f = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  // Which frame this CTA takes: CTAs are handed out in index order, one per SM, so CTA i takes the frame with the
+  // i-th largest survivor count — the long frames start in the first wave and the tail is made of short ones.
+  __shared__ int s_frame;
+  {
+    const int B = (int)gridDim.x, i = (int)blockIdx.x;
+    if (B <= sm_count || B > K2_MAXPERM) {
+      if (tid == 0) s_frame = i;
+    } else {
+      int* wts = reinterpret_cast<int*>(cnt);                      // the counter array is free until the select
+      for (int g = tid; g < B; g += K2_THREADS) wts[g] = surv_cnt[g];
+      __syncthreads();
+      for (int g = tid; g < B; g += K2_THREADS) {
+        const int wg = wts[g];
+        int rank = 0;
+        for (int h = 0; h < B; ++h) { const int wh = wts[h]; rank += (wh > wg) | ((wh == wg) & (h < g)); }
+        if (rank == i) s_frame = g;
+      }
+    }
+    __syncthreads();
+  }
+  const int f = s_frame;
   if (tid == 0) { fd = frames[f]; misc->counter = 0; }
   __syncthreads();
   const int n = surv_cnt[f];
@@ -427,21 +449,31 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
   // over the L2-resident keys instead of one shared atomic per warp step on a single hot counter) ----
   {
     int mine = 0;
-    for (int base = warp * 32; base < n; base += K2_THREADS) {
-      const int i = base + lane;
-      mine += __popc(__ballot_sync(0xffffffffu, i < n && gk[i] <= thr));
+    for (int base = warp * 32; base < n; base += 4 * K2_THREADS) {
+      KeyT key[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) { const int i = base + u * K2_THREADS + lane; key[u] = i < n ? gk[i] : ~(KeyT)0; }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int i = base + u * K2_THREADS + lane;
+        mine += __popc(__ballot_sync(0xffffffffu, i < n && key[u] <= thr));
+      }
     }
     int total;
     const int inc = blk_scan_inclusive(lane == 0 ? mine : 0, misc, 0, tid, &total);
     int at = __shfl_sync(0xffffffffu, inc, 0) - mine;            // first slot of this warp
-    for (int base = warp * 32; base < n; base += K2_THREADS) {
-      const int i = base + lane;
-      KeyT key = 0;
-      bool m = false;
-      if (i < n) { key = gk[i]; m = key <= thr; }
-      const uint32_t bal = __ballot_sync(0xffffffffu, m);
-      if (m) sel[at + __popc(bal & ((1u << lane) - 1u))] = key;
-      at += __popc(bal);
+    for (int base = warp * 32; base < n; base += 4 * K2_THREADS) {
+      KeyT key[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) { const int i = base + u * K2_THREADS + lane; key[u] = i < n ? gk[i] : ~(KeyT)0; }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int i = base + u * K2_THREADS + lane;
+        const bool m = i < n && key[u] <= thr;
+        const uint32_t bal = __ballot_sync(0xffffffffu, m);
+        if (m) sel[at + __popc(bal & ((1u << lane) - 1u))] = key[u];
+        at += __popc(bal);
+      }
     }
   }
   for (int i = tid; i < K2_CNT_WORDS; i += K2_THREADS) cnt[i] = 0u;
@@ -462,7 +494,9 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
         while (l + 1 < cst.num_levels && idx >= fd.lvl_start[l + 1]) ++l;
         const int k = idx - fd.lvl_start[l];
         const int gw = fd.lvl_gw[l];
-        const int iy = k / gw, ix = k - iy * gw;
+        int iy = (int)(((float)k + 0.5f) * __frcp_rn((float)gw));        // k < 2^20: off by at most one, fixed below
+        int ix = k - iy * gw;
+        if (ix < 0) { --iy; ix += gw; } else if (ix >= gw) { ++iy; ix -= gw; }
         const float s = (float)(1 << cst.stride_log2[l]);
         ps[u][0] = __fmul_rn((float)ix + 0.5f, s); ps[u][1] = __fmul_rn((float)iy + 0.5f, s); ps[u][2] = s;
         const int64_t row = fd.cand_off + idx;
