@@ -879,8 +879,10 @@ __global__ void __launch_bounds__(K4_THREADS, 2) k4_resolve_emit(
   K4Misc* misc = reinterpret_cast<K4Misc*>(hist + K4_WARPS * 256);
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  // Which frame this CTA takes.  All CTAs start at once, two per SM, and the hardware hands out CTAs 0..S-1 one per
-  // SM before it doubles up: give those the S heaviest frames (heaviest first) and pair them with the lightest ones.
+  // Which frame this CTA takes.  All CTAs start at once; the hardware hands out CTAs 0..S-1 one per SM and then CTA
+  // S+j to the SM of CTA j (checked with %smid), so with B < 2S frames the SMs of CTAs B-S..S-1 run ONE frame.  The
+  // frames are ranked by an estimate of their a4 time (edges, boxes, and the kept count the edge count implies); the
+  // 2S-B longest run alone, the next longest are paired with the shortest.
   __shared__ int s_w[K4_MAXPERM];
   __shared__ int s_frame;
   {
@@ -888,9 +890,18 @@ __global__ void __launch_bounds__(K4_THREADS, 2) k4_resolve_emit(
     if (B <= S || B > K4_MAXPERM) {
       if (tid == 0) s_frame = i;
     } else {
-      for (int g = tid; g < B; g += K4_THREADS) s_w[g] = edge_ctr[g] + 3 * n_sorted[g];
+      for (int g = tid; g < B; g += K4_THREADS) {
+        const int ng = n_sorted[g], eg = edge_ctr[g];
+        const int kept_est = ng - eg / 5 > ng / 10 ? ng - eg / 5 : ng / 10;
+        s_w[g] = eg / 2 + 9 * kept_est + 3 * ng;
+      }
       __syncthreads();
-      const int want = i < S ? i : (i < 2 * S ? B - 1 - (i - S) : S + (i - 2 * S));     // rank in descending weight
+      const int alone = 2 * S - B > 0 ? 2 * S - B : 0;             // SMs that get a single CTA
+      int want;                                                    // rank in descending weight
+      if (i >= S) want = i < 2 * S ? B - 1 - (i - S) : alone + (i - S);   // second CTA of an SM: shortest first
+      else if (i >= S - alone) want = i - (S - alone);             // alone on its SM: the longest frames
+      else want = alone + i;                                       // first CTA of a shared SM
+      if (B >= 2 * S) want = i < S ? i : (i < 2 * S ? B - 1 - (i - S) : S + (i - 2 * S));
       for (int g = tid; g < B; g += K4_THREADS) {
         const int wg = s_w[g];
         int rank = 0;
