@@ -83,7 +83,7 @@ int ffpp_create(const ffpp_params* p /*HOST*/, ffpp_handle** out /*HOST*/);
  *   frame_dims   HOST    [B][2] = (W, H) pixels; W a multiple of the largest stride and of cell_px, H a multiple
  *                        of cell_px, W*H a multiple of s_l^2 for every level.  Read before return.
  *   stream       cudaStream_t (as void*); NULL = legacy default stream.
- *   out_boxes    DEVICE  [B][top_k] ffpp_box; rows [0, out_counts[f]) of frame f are valid, in keep order
+ *   out_boxes    DEVICE  [B][top_k] ffpp_box, 8-byte aligned base; rows [0, out_counts[f]) of frame f are valid, in keep order
  *                        (= score order); the rest is left untouched.
  *   out_counts   DEVICE  [B] int32: boxes kept by NMS (in-frame or not, A19).
  *   out_density  DEVICE  float32, per-frame row-major [H/cell][W/cell] grids concatenated in frame order; every

@@ -327,6 +327,7 @@ int ffpp_create(const ffpp_params* p, ffpp_handle** out) {
   c.num_levels = p->num_levels;
   for (int l = 0; l < p->num_levels; ++l) c.stride_log2[l] = ilog2(p->strides[l]);
   c.cell_px = p->cell_px;
+  c.cell_inv = is_pow2(p->cell_px) ? 1.0f / (float)p->cell_px : 0.0f;
   c.radius = R;
   {
     double Z = 0.0, s2 = 2.0 * (double)p->sigma_cells * (double)p->sigma_cells;
@@ -413,6 +414,7 @@ int ffpp_run(ffpp_handle* h, const void* raw, int32_t B, const int32_t* N_per_fr
   if (!raw || !N_per_frame || !frame_dims || !out_boxes || !out_counts || !out_density) return fail(h, FFPP_EINVAL, "null pointer");
   if (B > h->p.max_frames) return fail(h, FFPP_ECAPACITY, "B exceeds max_frames");
   if (reinterpret_cast<uintptr_t>(raw) & 15) return fail(h, FFPP_EINVAL, "raw must be 16-byte aligned");
+  if (reinterpret_cast<uintptr_t>(out_boxes) & 7) return fail(h, FFPP_EINVAL, "out_boxes must be 8-byte aligned");
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   if (h->timing) FFPP_CUDA(h, cudaEventRecord(h->ev[0], st));
   int rc = schedule(h, B, N_per_frame, frame_dims, st);

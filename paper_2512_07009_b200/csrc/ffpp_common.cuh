@@ -43,6 +43,7 @@ struct Consts {
   int32_t num_levels;
   int32_t stride_log2[kMaxLevels];
   int32_t cell_px;
+  float cell_inv;                   // 1 / cell_px if cell_px is a power of two (the product is then exact), else 0
   int32_t radius;
   float taps[2 * kMaxRadius + 1];
   int32_t radius_t;                 // compile-time radius bucket RT >= radius that a6 runs with
@@ -136,17 +137,18 @@ __device__ __forceinline__ bool iou_exceeds(const float4 a, const float4 b, cons
 // global cell number dens_off + cy*gw + cx; the 32-bit atomicAdd on the containing word cannot carry between halves.
 __device__ __forceinline__ void emit_kept(const FrameDesc& fd, const Consts& cst, ffpp_box* __restrict__ dst, const float4 bx,
                                           const float logit, const int idx, uint32_t* __restrict__ hist32) {
-  ffpp_box o;
-  o.x1 = bx.x; o.y1 = bx.y; o.x2 = bx.z; o.y2 = bx.w;
-  o.score = __fdiv_rn(1.0f, __fadd_rn(1.0f, expf(-logit)));
-  o.cand_index = idx;
-  *dst = o;
+  const float score = __fdiv_rn(1.0f, __fadd_rn(1.0f, expf(-logit)));
+  float2* d2 = reinterpret_cast<float2*>(dst);                 // a record is 24 bytes, rows start 8-byte aligned
+  d2[0] = make_float2(bx.x, bx.y);
+  d2[1] = make_float2(bx.z, bx.w);
+  d2[2] = make_float2(score, __int_as_float(idx));
   const float cx = __fmul_rn(__fadd_rn(bx.x, bx.z), 0.5f);
   const float cy = __fmul_rn(__fadd_rn(bx.y, bx.w), 0.5f);
   if (cx >= 0.0f && cx < (float)fd.W && cy >= 0.0f && cy < (float)fd.H) {
     const float cell = (float)cst.cell_px;
-    const int cxi = (int)floorf(__fdiv_rn(cx, cell));
-    const int cyi = (int)floorf(__fdiv_rn(cy, cell));
+    // cell_inv != 0: cell_px is a power of two, x * (1/cell) IS the correctly rounded x / cell
+    const int cxi = (int)floorf(cst.cell_inv != 0.0f ? __fmul_rn(cx, cst.cell_inv) : __fdiv_rn(cx, cell));
+    const int cyi = (int)floorf(cst.cell_inv != 0.0f ? __fmul_rn(cy, cst.cell_inv) : __fdiv_rn(cy, cell));
     const int64_t h = fd.dens_off + (int64_t)cyi * fd.gw + cxi;
     atomicAdd(&hist32[h >> 1], 1u << (16 * (int)(h & 1)));
   }
