@@ -812,10 +812,12 @@ __device__ __forceinline__ bool k4_lsd_pass(const KeyT* ksrc, const uint16_t* ps
   for (int base = w_begin; base < w_end; base += 32) {
     const int i = base + lane;
     const bool v = i < w_end;
-    const uint32_t dg = v ? (uint32_t)((ksrc[i] >> shift) & 255) : 0u;
-    const uint32_t peers = k4_peers8(dg, v);
-    // two uint16 counters per word; no carry (a warp segment has < 65536 entries)
-    if (v && lane == __ffs(peers) - 1) atomicAdd(&hist32[(warp * 256 + dg) >> 1], (uint32_t)__popc(peers) << (16 * (dg & 1)));
+    // two uint16 counters per word, one row per warp; no carry (a warp segment has < 65536 entries).  Counting needs
+    // no peer mask: same-digit lanes simply serialise on the shared atomic.
+    if (v) {
+      const uint32_t dg = (uint32_t)((ksrc[i] >> shift) & 255);
+      atomicAdd(&hist32[(warp * 256 + dg) >> 1], 1u << (16 * (dg & 1)));
+    }
   }
   __syncthreads();
   // thread d < 256 owns digit d: counts of the 16 warps, exclusive offsets in (digit major, warp minor) order
