@@ -205,15 +205,14 @@ __global__ void __launch_bounds__(K1_THREADS) k1_threshold_compact(const uint8_t
 }
 
 // =====================================================================================================
-// Block-wide (1024-thread) helpers shared by a2 and a4: exclusive scans and a stable 8-bit LSD radix pass.
+// Block-wide (1024-thread) helper of a2: inclusive scan of one int per thread.
 // =====================================================================================================
 constexpr int BLK_THREADS = 1024;
 constexpr int BLK_WARPS = BLK_THREADS / 32;
 
 struct BlkMisc {
   int wsum[2][BLK_WARPS];
-  int sel_digit, sel_kk, sel_tot, skip;
-  int counter;
+  int sel_digit, sel_kk, sel_tot;
 };
 
 // inclusive scan of one int per thread over the CTA; returns the inclusive value, *total = sum over the CTA.
@@ -233,84 +232,6 @@ __device__ __forceinline__ int blk_scan_inclusive(int v, BlkMisc* misc, int par,
   *total = __shfl_sync(0xffffffffu, winc, 31);
   __syncthreads();
   return before + inc;
-}
-
-__device__ __forceinline__ void blk_zero_hist(uint16_t* hist, int tid) {
-  uint32_t* h32 = reinterpret_cast<uint32_t*>(hist);
-  for (int i = tid; i < BLK_WARPS * 256 / 2; i += BLK_THREADS) h32[i] = 0;
-}
-
-// exclusive scan of the per-warp digit histogram hist[warp][digit] in (digit major, warp minor) order, in place.
-__device__ __forceinline__ void blk_scan_hist(uint16_t* hist, BlkMisc* misc, int tid) {
-  const int lane = tid & 31, warp = tid >> 5;
-  const int d = tid >> 2, w0 = (tid & 3) * 8;
-  int v[8], sum = 0;
-#pragma unroll
-  for (int j = 0; j < 8; ++j) { v[j] = hist[(w0 + j) * 256 + d]; sum += v[j]; }
-  int inc = sum;
-#pragma unroll
-  for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
-  if (lane == 31) misc->wsum[0][warp] = inc;
-  __syncthreads();
-  if (warp == 0) {
-    int x = misc->wsum[0][lane], xi = x;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, xi, o); if (lane >= o) xi += t; }
-    misc->wsum[0][lane] = xi - x;
-  }
-  __syncthreads();
-  int run = misc->wsum[0][warp] + inc - sum;
-#pragma unroll
-  for (int j = 0; j < 8; ++j) { hist[(w0 + j) * 256 + d] = (uint16_t)run; run += v[j]; }
-}
-
-// One stable LSD pass on the 8-bit digit at `shift` (per-warp contiguous segments ranked with match_any).
-// Returns true if the keys moved to dst (false: the digit is constant, nothing to reorder).
-template <typename T>
-__device__ __forceinline__ bool blk_lsd_pass(const T* src, T* dst, int n, int shift, uint16_t* hist, BlkMisc* misc, int tid) {
-  const int lane = tid & 31, warp = tid >> 5;
-  const int seg = ((n + BLK_WARPS - 1) / BLK_WARPS + 31) & ~31;    // per-warp contiguous segment
-  const int w_begin = warp * seg < n ? warp * seg : n;
-  const int w_end = (warp + 1) * seg < n ? (warp + 1) * seg : n;
-  uint32_t* hist32 = reinterpret_cast<uint32_t*>(hist);
-  blk_zero_hist(hist, tid);
-  if (tid == 0) misc->skip = 0;
-  __syncthreads();
-  for (int base = w_begin; base < w_end; base += 32) {
-    const int i = base + lane;
-    const bool v = i < w_end;
-    const uint32_t dg = v ? (uint32_t)((src[i] >> shift) & 255) : 256u;
-    const uint32_t peers = __match_any_sync(0xffffffffu, dg);
-    // two uint16 counters per word; fire-and-forget shared atomics, no carry (a warp segment has < 65536 keys)
-    if (v && lane == __ffs(peers) - 1) atomicAdd(&hist32[(warp * 256 + dg) >> 1], (uint32_t)__popc(peers) << (16 * (dg & 1)));
-  }
-  __syncthreads();
-  if (tid < 256) {
-    int s = 0;
-#pragma unroll 8
-    for (int w = 0; w < BLK_WARPS; ++w) s += hist[w * 256 + tid];
-    if (s == n) misc->skip = 1;
-  }
-  __syncthreads();
-  if (misc->skip) { __syncthreads(); return false; }
-  blk_scan_hist(hist, misc, tid);
-  __syncthreads();
-  for (int base = w_begin; base < w_end; base += 32) {
-    const int i = base + lane;
-    const bool v = i < w_end;
-    T key = 0;
-    if (v) key = src[i];
-    const uint32_t dg = v ? (uint32_t)((key >> shift) & 255) : 256u;
-    const uint32_t peers = __match_any_sync(0xffffffffu, dg);
-    int b = 0;
-    if (v) b = hist[warp * 256 + dg];
-    __syncwarp();
-    if (v && lane == __ffs(peers) - 1) hist[warp * 256 + dg] = (uint16_t)(b + __popc(peers));
-    __syncwarp();
-    if (v) dst[b + __popc(peers & ((1u << lane) - 1u))] = key;
-  }
-  __syncthreads();
-  return true;
 }
 
 // =====================================================================================================
@@ -378,7 +299,7 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
     __syncthreads();
   }
   const int f = s_frame;
-  if (tid == 0) { fd = frames[f]; misc->counter = 0; }
+  if (tid == 0) fd = frames[f];
   __syncthreads();
   const int n = surv_cnt[f];
   const int nsel = n < K ? n : K;
@@ -768,7 +689,8 @@ __host__ __device__ inline size_t k4_tail_bytes(size_t kpad) {
 // sort arrays for m kept boxes: two (key, position) buffers, m rounded up to a power of two for the bitonic path
 __host__ __device__ inline size_t k4_sort_bytes(size_t m, size_t key_bytes) {
   const size_t lsd = 2 * (((m * key_bytes + 15) & ~(size_t)15) + ((m * 2 + 15) & ~(size_t)15));
-  const size_t bit = m <= (size_t)K4_BITONIC_MAX ? k4_pow2ceil(m) * (key_bytes + 2) : 0;
+  const size_t np = k4_pow2ceil(m);                            // bitonic path: two buffers of pow2ceil(m) pairs
+  const size_t bit = m <= (size_t)K4_BITONIC_MAX ? 2 * (((np * key_bytes + 15) & ~(size_t)15) + ((np * 2 + 15) & ~(size_t)15)) : 0;
   return lsd > bit ? lsd : bit;
 }
 __host__ __device__ inline size_t k4_union_bytes(size_t top_k, size_t kpad, size_t key_bytes) {
@@ -857,6 +779,73 @@ __device__ __forceinline__ bool k4_lsd_pass(const KeyT* ksrc, const uint16_t* ps
   }
   __syncthreads();
   return true;
+}
+
+// Bitonic sort of m <= K4_BITONIC_MAX (key, position) pairs held in kA/pA (capacity Np = pow2ceil(m)); kB/pB is a second
+// buffer of the same size.  A thread keeps two elements in registers (e0 = 64 warp + lane, e1 = e0 + 32): partner
+// distances below 32 are shuffles, 32 is the thread's own pair, and only distances >= 64 go through shared memory —
+// 10 block barriers for 1024 keys instead of 55 (a barrier-bound sort crawls when another frame shares the SM).
+template <typename KeyT>
+__device__ __forceinline__ void k4_bitonic(KeyT* kA, uint16_t* pA, KeyT* kB, uint16_t* pB, const int m, const int Np, const int tid) {
+  const int lane = tid & 31, warp = tid >> 5;
+  const int e0 = warp * 64 + lane, e1 = e0 + 32;
+  const int NE = Np < 64 ? 64 : Np;
+  const bool part = e0 < NE;                                   // warp-uniform
+  KeyT k0 = ~(KeyT)0, k1 = ~(KeyT)0;                           // padding: maximal keys, sorted to the end, never stored
+  uint16_t q0 = 0, q1 = 0;
+  if (part) {
+    if (e0 < m) { k0 = kA[e0]; q0 = pA[e0]; }
+    if (e1 < m) { k1 = kA[e1]; q1 = pA[e1]; }
+  }
+  KeyT* xk[2] = {kB, kA};
+  uint16_t* xq[2] = {pB, pA};
+  int cur = 0;
+  __syncthreads();                                              // kA is free to be an exchange buffer from here on
+  for (int k = 2; k <= NE; k <<= 1) {
+    for (int j = k >> 1; j > 0; j >>= 1) {
+      if (j >= 64) {
+        KeyT* bk = cur ? xk[1] : xk[0];
+        uint16_t* bq = cur ? xq[1] : xq[0];
+        if (part) { bk[e0] = k0; bq[e0] = q0; bk[e1] = k1; bq[e1] = q1; }
+        __syncthreads();
+        if (part) {
+          {
+            const KeyT ok = bk[e0 ^ j]; const uint16_t oq = bq[e0 ^ j];
+            const bool take_min = ((e0 & j) == 0) == ((e0 & k) == 0);
+            if (take_min ? ok < k0 : ok > k0) { k0 = ok; q0 = oq; }
+          }
+          {
+            const KeyT ok = bk[e1 ^ j]; const uint16_t oq = bq[e1 ^ j];
+            const bool take_min = ((e1 & j) == 0) == ((e1 & k) == 0);
+            if (take_min ? ok < k1 : ok > k1) { k1 = ok; q1 = oq; }
+          }
+        }
+        cur ^= 1;
+      } else if (part) {
+        if (j == 32) {
+          if ((k0 > k1) == ((e0 & k) == 0)) { const KeyT tk = k0; k0 = k1; k1 = tk; const uint16_t tq = q0; q0 = q1; q1 = tq; }
+        } else {
+          const bool lower = (lane & j) == 0;
+          {
+            const KeyT ok = __shfl_xor_sync(0xffffffffu, k0, j); const uint16_t oq = (uint16_t)__shfl_xor_sync(0xffffffffu, (int)q0, j);
+            const bool take_min = lower == ((e0 & k) == 0);
+            if (take_min ? ok < k0 : ok > k0) { k0 = ok; q0 = oq; }
+          }
+          {
+            const KeyT ok = __shfl_xor_sync(0xffffffffu, k1, j); const uint16_t oq = (uint16_t)__shfl_xor_sync(0xffffffffu, (int)q1, j);
+            const bool take_min = lower == ((e1 & k) == 0);
+            if (take_min ? ok < k1 : ok > k1) { k1 = ok; q1 = oq; }
+          }
+        }
+      }
+    }
+  }
+  __syncthreads();                                              // every exchange read is done
+  if (part) {
+    if (e0 < m) { kA[e0] = k0; pA[e0] = q0; }
+    if (e1 < m) { kA[e1] = k1; pA[e1] = q1; }
+  }
+  __syncthreads();
 }
 
 template <typename KeyT>
@@ -1043,24 +1032,10 @@ __global__ void __launch_bounds__(K4_THREADS, 2) k4_resolve_emit(
       }
     }
   }
-  if (bitonic)
-    for (int i = m + tid; i < Np; i += K4_THREADS) { kk[i] = ~(KeyT)0; pp[i] = 0; }
   __syncthreads();
   FFPP_PHASE(f, 4);
   if (bitonic) {
-    for (int k = 2; k <= Np; k <<= 1) {
-      for (int j = k >> 1; j > 0; j >>= 1) {
-        for (int t = tid; t < (Np >> 1); t += K4_THREADS) {
-          const int i = ((t & ~(j - 1)) << 1) | (t & (j - 1)), l = i | j;
-          const KeyT ka = kk[i], kb = kk[l];
-          if ((ka > kb) == ((i & k) == 0)) {
-            kk[i] = kb; kk[l] = ka;
-            const uint16_t t0 = pp[i]; pp[i] = pp[l]; pp[l] = t0;
-          }
-        }
-        __syncthreads();
-      }
-    }
+    k4_bitonic<KeyT>(kk, pp, kk1, pp1, m, Np, tid);
   } else {
     for (int shift = 0; shift < KB; shift += 8)
       if (k4_lsd_pass<KeyT>(kk, pp, kk1, pp1, m, shift, hist, misc, tid)) {
