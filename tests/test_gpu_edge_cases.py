@@ -127,6 +127,18 @@ def test_many_tiny_frames_take_the_generic_compaction_path(env):
     check(env, w)
 
 
+@pytest.mark.parametrize("B", [297, 400, 1100])
+def test_more_frames_than_resident_ctas(env, B):
+    """B above 2 x SM count (a4's CTAs no longer all start at once) and above the 1024-frame limit of the
+    weight-ordered CTA -> frame maps of a2 / a4 (identity map)."""
+    torch, m, oracle_mod, gen = env
+    rng = np.random.default_rng(B)
+    dims = [[64, 64] if i % 3 else [128, 64] for i in range(B)]
+    parts = [frame(gen.frame_candidates(a, b), np.float16, rng, int(rng.integers(0, 70)), lo=0.0, hi=8.0) for a, b in dims]
+    w = W(np.concatenate(parts), dims, dict(P, top_k=40, sigma_cells=1.0))
+    check(env, w)
+
+
 def test_max_topk_for_both_key_widths(env):
     rng = np.random.default_rng(8)
     N = 42840
