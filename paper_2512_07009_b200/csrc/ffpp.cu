@@ -84,10 +84,10 @@ struct ffpp_handle {
   cudaEvent_t ev[FFPP_NUM_STAGES + 1] = {};
   bool ev_valid = false;
 
-  int* surv_cnt() const { return d_counters; }
-  int* n_sorted() const { return d_counters + p.max_frames; }
-  int* edge_ctr() const { return d_counters + 2 * (size_t)p.max_frames; }
-  int* frame_err() const { return d_counters + 3 * (size_t)p.max_frames; }
+  int* n_sorted() const { return d_counters; }
+  int* edge_ctr() const { return d_counters + (size_t)p.max_frames; }
+  int* frame_err() const { return d_counters + 2 * (size_t)p.max_frames; }
+  int* surv_cnt() const { return d_counters + 3 * (size_t)p.max_frames; }     // kCntStride ints per frame
 };
 
 namespace {
@@ -369,7 +369,7 @@ int ffpp_create(const ffpp_params* p, ffpp_handle** out) {
   const size_t KP = (size_t)h->kpad, F = (size_t)p->max_frames;
   if ((e = dalloc((void**)&h->d_meta, h->ml.bytes)) != cudaSuccess ||
       (e = dalloc(&h->d_surv_keys, (size_t)p->max_total_candidates * h->key_bytes)) != cudaSuccess ||
-      (e = dalloc((void**)&h->d_counters, 4 * F * sizeof(int))) != cudaSuccess ||
+      (e = dalloc((void**)&h->d_counters, (3 + kCntStride) * F * sizeof(int))) != cudaSuccess ||
       (e = dalloc((void**)&h->d_sel_box, F * KP * sizeof(float4))) != cudaSuccess ||
       (e = dalloc((void**)&h->d_sp_box, F * KP * sizeof(float4))) != cudaSuccess ||
       (e = dalloc((void**)&h->d_sp_sbox, F * KP * sizeof(float4))) != cudaSuccess ||
@@ -419,7 +419,7 @@ int ffpp_run(ffpp_handle* h, const void* raw, int32_t B, const int32_t* N_per_fr
   if (h->timing) FFPP_CUDA(h, cudaEventRecord(h->ev[0], st));
   int rc = schedule(h, B, N_per_frame, frame_dims, st);
   if (rc != FFPP_OK) return rc;
-  FFPP_CUDA(h, cudaMemsetAsync(h->d_counters, 0, sizeof(int) * 4 * (size_t)h->p.max_frames, st));
+  FFPP_CUDA(h, cudaMemsetAsync(h->d_counters, 0, sizeof(int) * (3 + kCntStride) * (size_t)h->p.max_frames, st));
   if (h->half && h->key_bytes == 4) return launch_all<true, uint32_t>(h, raw, B, st, out_boxes, out_counts, out_density);
   if (h->half) return launch_all<true, uint64_t>(h, raw, B, st, out_boxes, out_counts, out_density);
   return launch_all<false, uint64_t>(h, raw, B, st, out_boxes, out_counts, out_density);
@@ -530,7 +530,10 @@ int ffpp_debug_read(ffpp_handle* h, int32_t what, void* dst, int64_t dst_bytes) 
   FFPP_CUDA(h, cudaDeviceSynchronize());
   if (what == 0 || what == 1) {
     if (dst_bytes < (int64_t)(sizeof(int) * B)) return fail(h, FFPP_EINVAL, "dst too small");
-    FFPP_CUDA(h, cudaMemcpy(dst, what == 0 ? h->surv_cnt() : h->n_sorted(), sizeof(int) * B, cudaMemcpyDeviceToHost));
+    if (what == 0)
+      FFPP_CUDA(h, cudaMemcpy2D(dst, sizeof(int), h->surv_cnt(), sizeof(int) * kCntStride, sizeof(int), (size_t)B, cudaMemcpyDeviceToHost));
+    else
+      FFPP_CUDA(h, cudaMemcpy(dst, h->n_sorted(), sizeof(int) * B, cudaMemcpyDeviceToHost));
     return FFPP_OK;
   }
   if (what != 2 && what != 3) return fail(h, FFPP_EINVAL, "unknown debug selector");

@@ -12,6 +12,8 @@ constexpr int kMaxLevels = 4;
 constexpr int kMaxRadius = 32;
 constexpr int kBlk = 32;            // kpad granularity
 constexpr int kMaxTopK = 24576;     // positions fit 15 bits (adjacency entries carry one more bit)
+constexpr int kCntStride = 32;      // ints between two frames' survivor counters: one 128-byte line each, so the a1 atomics
+                                    // of different frames go to different L2 lines
 constexpr int kMaxCells = 16384;    // spatial cells per frame (<= 128 x 128)
 constexpr int kCellStride = kMaxCells + 8;   // uint16 entries per frame in the cell-start table
 

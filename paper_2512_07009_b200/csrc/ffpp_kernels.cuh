@@ -110,14 +110,21 @@ __global__ void __launch_bounds__(K1_THREADS) k1_threshold_compact(const uint8_t
       p_total = 0;
     }
   };
+  // table entries of this warp's first 32 slices, one per lane, fetched before the loop (a dependent global load per
+  // slice would sit on the critical path of every iteration); later slices, if any, look the table up in the loop
+  int bf_lane = 0;
+  {
+    const int64_t g = ((int64_t)blockIdx.x + (int64_t)lane * gridDim.x) * CPC + (int64_t)warp * CPW;
+    if (g < total_cand) bf_lane = block_frame[g / K1_BLOCK];
+  }
   int it = 0;
   for (int64_t c = blockIdx.x; c < nchunks; c += gridDim.x, ++it) {
     const int stage = it % K1_STAGES;
     const uint8_t* buf = ring + (size_t)stage * K1_CHUNK_BYTES;
     const int64_t gw0 = c * CPC + (int64_t)warp * CPW;          // first candidate of this warp's slice
     int f0 = 0;
-    if (gw0 < total_cand) {                                     // frame of gw0 (overlaps the copy): table + short walk
-      f0 = block_frame[gw0 / K1_BLOCK];
+    if (gw0 < total_cand) {                                     // frame of gw0: table + short walk in shared memory
+      f0 = it < 32 ? __shfl_sync(0xffffffffu, bf_lane, it) : block_frame[gw0 / K1_BLOCK];
       while (coff[f0 + 1] <= gw0) ++f0;
     }
     mbar_wait(&full[stage], (uint32_t)(it / K1_STAGES) & 1u);
@@ -154,7 +161,7 @@ __global__ void __launch_bounds__(K1_THREADS) k1_threshold_compact(const uint8_t
       const int total = __shfl_sync(0xffffffffu, inc, 31);
       flush_pending();                                          // the previous slice: its atomic has had a whole chunk to return
       if (total) {
-        if (lane == 31) p_base = atomicAdd(&surv_cnt[f0], total);   // not consumed until the next flush
+        if (lane == 31) p_base = atomicAdd(&surv_cnt[f0 * kCntStride], total);   // not consumed until the next flush
         p_total = total; p_pass = pass; p_excl = inc - c; p_coff = coff[f0];
 #pragma unroll
         for (int i = 0; i < CPL; ++i) p_keys[i] = keys[i];
@@ -190,7 +197,7 @@ __global__ void __launch_bounds__(K1_THREADS) k1_threshold_compact(const uint8_t
         }
         if (cnt == 0) continue;
         int base = 0;
-        if (lane == 0) base = atomicAdd(&surv_cnt[f], cnt);
+        if (lane == 0) base = atomicAdd(&surv_cnt[f * kCntStride], cnt);
         base = __shfl_sync(0xffffffffu, base, 0);
         KeyT* dst = surv_keys + coff[f] + base;
 #pragma unroll
@@ -287,7 +294,7 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
       if (tid == 0) s_frame = i;
     } else {
       int* wts = reinterpret_cast<int*>(cnt);                      // the counter array is free until the select
-      for (int g = tid; g < B; g += K2_THREADS) wts[g] = surv_cnt[g];
+      for (int g = tid; g < B; g += K2_THREADS) wts[g] = surv_cnt[g * kCntStride];
       __syncthreads();
       for (int g = tid; g < B; g += K2_THREADS) {
         const int wg = wts[g];
@@ -301,7 +308,7 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
   const int f = s_frame;
   if (tid == 0) fd = frames[f];
   __syncthreads();
-  const int n = surv_cnt[f];
+  const int n = surv_cnt[f * kCntStride];
   const int nsel = n < K ? n : K;
   const KeyT* gk = surv_keys + fd.cand_off;
 
