@@ -352,11 +352,15 @@ def run_ours(args):
         roofline["stage"] = names[dom]
         roofline["avg_launch_ms"] = float(stage_ms[dom])
         roofline["hbm_peak_source"] = peak_src
-        tr_path = os.path.join(ROOT, "profiles", f"traffic_config{c}.json")
+        tr_path = os.path.join(ROOT, "profiles", f"traffic_config{c}.csv")
         if os.path.exists(tr_path):      # per-launch numbers of the committed ncu --set full capture of this config
-            with open(tr_path) as fh:
-                tr = json.load(fh)
-            k = tr.get("kernels", {}).get(roofline["kernel"])
+            import csv
+            with open(tr_path, newline="") as fh:
+                rows = {r["kernel"]: r for r in csv.DictReader(fh)}
+            k = rows.get(roofline["kernel"])
+            if k:
+                k = {kk: float(vv) for kk, vv in k.items() if kk != "kernel"}
+            tr = {"source": "profiles/r1_v4_config5_config4_ncu.md (ncu --set full, one launch of each kernel, cold cache)"}
             if k:
                 roofline["traffic"] = k["dram_bytes"]            # dram__bytes_read.sum + dram__bytes_write.sum
                 roofline["traffic_source"] = tr.get("source")
