@@ -1120,9 +1120,13 @@ __global__ void __launch_bounds__(K5_THREADS) k5_density(const FrameDesc* __rest
   const FrameDesc* fd = &frames[f];
   const int gw = fd->gw, gh = fd->gh;
   const int tw = k5_tile_w(gw);
-  const int tiles_x = (gw + tw - 1) / tw, tiles_y = (gh + K5_TH - 1) / K5_TH;
-  if ((int)blockIdx.x >= tiles_x * tiles_y) return;
-  const int ty = blockIdx.x / tiles_x, tx = blockIdx.x - ty * tiles_x;
+  const int tiles_y = (gh + K5_TH - 1) / K5_TH;
+  int ty = (int)blockIdx.x, tx = 0;
+  if (gw > tw) {                                            // grids wider than one tile (> K5_TW columns) only
+    const int tiles_x = (gw + tw - 1) / tw;
+    ty = (int)blockIdx.x / tiles_x; tx = (int)blockIdx.x - ty * tiles_x;
+  }
+  if (ty >= tiles_y) return;
   const int x0 = tx * tw, y0 = ty * K5_TH;
   const int P = k5_pitch(tw, RT);
   const int twh = tw + 2 * RT;
@@ -1130,10 +1134,10 @@ __global__ void __launch_bounds__(K5_THREADS) k5_density(const FrameDesc* __rest
   const uint16_t* hsrc = hist16 + fd->dens_off;
   constexpr int NW = 8 + 2 * RT;                            // window of one 8-output block
 
-  // ---- y pass: unit = (column c, 8-row block q) ----
-  for (int u = tid; u < twh * (K5_TH / 8); u += K5_THREADS) {
-    const int q = u / twh, c = u - q * twh;
-    const int gx = k5_fold(x0 - RT + c, gw);
+  // ---- y pass: a thread owns column c and walks the strip's 8-row blocks ----
+  for (int c = tid; c < twh; c += K5_THREADS) {
+   const int gx = k5_fold(x0 - RT + c, gw);
+   for (int q = 0; q < K5_TH / 8; ++q) {
     const int yb = y0 + 8 * q - RT;
     float acc[8];
 #pragma unroll
@@ -1163,6 +1167,7 @@ __global__ void __launch_bounds__(K5_THREADS) k5_density(const FrameDesc* __rest
     }
 #pragma unroll
     for (int m = 0; m < 8; ++m) s_t[(8 * q + m) * P + c] = acc[m];
+   }
   }
   if (tid < 2 * K5_TH) s_t[(tid >> 1) * P + twh + (tid & 1)] = 0.0f;     // the two slack columns the float4 loads touch
   __syncthreads();
