@@ -95,7 +95,10 @@ int ffpp_run(ffpp_handle* h, const void* raw /*DEVICE*/, int32_t B, const int32_
 
 /* The same path with HOST buffers (the call a user without device buffers makes): copies raw host->device,
  * runs, copies the three outputs device->host through the handle's own staging, and synchronises `stream`
- * before returning.  raw / out_* are HOST pointers (pinned memory makes the copies asynchronous DMA). */
+ * before returning.  raw / out_* are HOST pointers (pinned memory makes the copies asynchronous DMA; a pinned
+ * out_boxes is written by one kernel through its device alias).  Batches of >= 32 MB and >= 16 frames are cut into
+ * four runs of whole frames (frames are independent) so that the upload of the next run and the download of the
+ * previous one, on two internal copy streams, overlap the kernels of the current run on `stream`. */
 int ffpp_run_host(ffpp_handle* h, const void* raw /*HOST*/, int32_t B, const int32_t* N_per_frame /*HOST*/,
                   const int32_t* frame_dims /*HOST*/, void* stream, ffpp_box* out_boxes /*HOST*/,
                   int32_t* out_counts /*HOST*/, float* out_density /*HOST*/);

@@ -79,6 +79,8 @@ struct ffpp_handle {
   ffpp_box* d_out_boxes = nullptr;
   int* d_out_counts = nullptr;
   float* d_out_density = nullptr;
+  cudaStream_t s_h2d = nullptr, s_d2h = nullptr;     // copy streams of the chunked host path (created on first use)
+  cudaEvent_t ev_up[4] = {}, ev_run[4] = {};
   // stage timing
   bool timing = false;
   cudaEvent_t ev[FFPP_NUM_STAGES + 1] = {};
@@ -448,9 +450,6 @@ int ffpp_run_host(ffpp_handle* h, const void* raw, int32_t B, const int32_t* N_p
   }
   if (cand > h->p.max_total_candidates) return fail(h, FFPP_ECAPACITY, "sum N_f exceeds max_total_candidates");
   if (cells > h->max_total_cells) return fail(h, FFPP_ECAPACITY, "density cells exceed max_total_cells");
-  FFPP_CUDA(h, cudaMemcpyAsync(h->d_in, raw, (size_t)cand * 5 * esz, cudaMemcpyHostToDevice, st));
-  int rc = ffpp_run(h, h->d_in, B, N_per_frame, frame_dims, stream, h->d_out_boxes, h->d_out_counts, h->d_out_density);
-  if (rc != FFPP_OK) return rc;
   // kept boxes: only rows [0, count) of each frame are defined.  A pinned (device-mapped) out_boxes is written by one
   // kernel through its device alias; a pageable one gets one copy per frame after the counts have arrived.
   const size_t K = (size_t)h->p.top_k;
@@ -462,12 +461,72 @@ int ffpp_run_host(ffpp_handle* h, const void* raw, int32_t B, const int32_t* N_p
     else
       cudaGetLastError();
   }
-  if (alias) {
-    const dim3 g((unsigned)std::min<size_t>(16, (K * 3 + KH_THREADS - 1) / KH_THREADS), (unsigned)B);
-    kh_copy_kept_rows<<<g, KH_THREADS, 0, st>>>(h->d_out_boxes, h->d_out_counts, (int)K, alias);
+  // Frames are independent, so a large batch is cut into up to kHostChunks runs of whole frames: the upload of run
+  // i+1 (copy stream) and the download of run i-1 (second copy stream) overlap the kernels of run i on `stream`.
+  // A run starts where the raw byte offset is a multiple of 16 (ffpp_run's alignment rule).
+  constexpr int kHostChunks = 4;
+  const size_t row = 5 * esz;
+  std::vector<int> cut{0};                                          // first frame of every run, then B
+  if (B >= 4 * kHostChunks && (size_t)cand * row >= ((size_t)32 << 20)) {
+    int64_t acc = 0;
+    int next = 1;
+    for (int f = 0; f < B && next < kHostChunks; ++f) {
+      if (f > cut.back() && acc * (int64_t)row % 16 == 0 && acc >= cand * next / kHostChunks) { cut.push_back(f); ++next; }
+      acc += N_per_frame[f];
+    }
   }
-  FFPP_CUDA(h, cudaMemcpyAsync(out_counts, h->d_out_counts, sizeof(int) * (size_t)B, cudaMemcpyDeviceToHost, st));
-  FFPP_CUDA(h, cudaMemcpyAsync(out_density, h->d_out_density, sizeof(float) * (size_t)cells, cudaMemcpyDeviceToHost, st));
+  cut.push_back(B);
+  const int C = (int)cut.size() - 1;
+  if (C > 1 && !h->s_h2d) {
+    FFPP_CUDA(h, cudaStreamCreateWithFlags(&h->s_h2d, cudaStreamNonBlocking));
+    FFPP_CUDA(h, cudaStreamCreateWithFlags(&h->s_d2h, cudaStreamNonBlocking));
+    for (int i = 0; i < kHostChunks; ++i) {
+      FFPP_CUDA(h, cudaEventCreateWithFlags(&h->ev_up[i], cudaEventDisableTiming));
+      FFPP_CUDA(h, cudaEventCreateWithFlags(&h->ev_run[i], cudaEventDisableTiming));
+    }
+  }
+  cudaStream_t s_up = C > 1 ? h->s_h2d : st, s_dn = C > 1 ? h->s_d2h : st;
+  if (C > 1) {                                                      // the copy streams start after what is already on `stream`
+    FFPP_CUDA(h, cudaEventRecord(h->ev_run[0], st));
+    FFPP_CUDA(h, cudaStreamWaitEvent(s_up, h->ev_run[0], 0));
+  }
+  std::vector<int64_t> c_off((size_t)C + 1, 0), d_off((size_t)C + 1, 0);
+  for (int i = 0; i < C; ++i) {
+    int64_t cc = 0, dd = 0;
+    for (int f = cut[(size_t)i]; f < cut[(size_t)i + 1]; ++f) {
+      cc += N_per_frame[f];
+      dd += (int64_t)(frame_dims[2 * f] / h->p.cell_px) * (frame_dims[2 * f + 1] / h->p.cell_px);
+    }
+    c_off[(size_t)i + 1] = c_off[(size_t)i] + cc;
+    d_off[(size_t)i + 1] = d_off[(size_t)i] + dd;
+  }
+  uint8_t* d_in8 = static_cast<uint8_t*>(h->d_in);
+  const uint8_t* raw8 = static_cast<const uint8_t*>(raw);
+  for (int i = 0; i < C; ++i)                                       // all uploads are queued up front, in order
+  {
+    const size_t o = (size_t)c_off[(size_t)i] * row, nbytes = (size_t)(c_off[(size_t)i + 1] - c_off[(size_t)i]) * row;
+    FFPP_CUDA(h, cudaMemcpyAsync(d_in8 + o, raw8 + o, nbytes, cudaMemcpyHostToDevice, s_up));
+    if (C > 1) FFPP_CUDA(h, cudaEventRecord(h->ev_up[i], s_up));
+  }
+  for (int i = 0; i < C; ++i) {
+    const int f0 = cut[(size_t)i], Bi = cut[(size_t)i + 1] - f0;
+    if (C > 1) FFPP_CUDA(h, cudaStreamWaitEvent(st, h->ev_up[i], 0));
+    const int rc = ffpp_run(h, d_in8 + (size_t)c_off[(size_t)i] * row, Bi, N_per_frame + f0, frame_dims + 2 * f0, stream,
+                            h->d_out_boxes + (size_t)f0 * K, h->d_out_counts + f0, h->d_out_density + d_off[(size_t)i]);
+    if (rc != FFPP_OK) { cudaStreamSynchronize(s_up); cudaStreamSynchronize(st); cudaStreamSynchronize(s_dn); return rc; }
+    if (C > 1) {
+      FFPP_CUDA(h, cudaEventRecord(h->ev_run[i], st));
+      FFPP_CUDA(h, cudaStreamWaitEvent(s_dn, h->ev_run[i], 0));
+    }
+    if (alias) {
+      const dim3 g((unsigned)std::min<size_t>(16, (K * 3 + KH_THREADS - 1) / KH_THREADS), (unsigned)Bi);
+      kh_copy_kept_rows<<<g, KH_THREADS, 0, s_dn>>>(h->d_out_boxes + (size_t)f0 * K, h->d_out_counts + f0, (int)K, alias + (size_t)f0 * K);
+    }
+    FFPP_CUDA(h, cudaMemcpyAsync(out_counts + f0, h->d_out_counts + f0, sizeof(int) * (size_t)Bi, cudaMemcpyDeviceToHost, s_dn));
+    FFPP_CUDA(h, cudaMemcpyAsync(out_density + d_off[(size_t)i], h->d_out_density + d_off[(size_t)i],
+                                 sizeof(float) * (size_t)(d_off[(size_t)i + 1] - d_off[(size_t)i]), cudaMemcpyDeviceToHost, s_dn));
+  }
+  FFPP_CUDA(h, cudaStreamSynchronize(s_dn));
   FFPP_CUDA(h, cudaStreamSynchronize(st));
   if (!alias) {
     for (int f = 0; f < B; ++f)
@@ -486,6 +545,9 @@ int ffpp_destroy(ffpp_handle* h) {
   cudaFree(h->d_sp_sbox); cudaFree(h->d_sp_key); cudaFree(h->d_cellstart); cudaFree(h->d_hasin); cudaFree(h->d_k4_scratch); cudaFree(h->d_edges);
   cudaFree(h->d_hist32);
   cudaFree(h->d_in); cudaFree(h->d_out_boxes); cudaFree(h->d_out_counts); cudaFree(h->d_out_density);
+  if (h->s_h2d) cudaStreamDestroy(h->s_h2d);
+  if (h->s_d2h) cudaStreamDestroy(h->s_d2h);
+  for (int i = 0; i < 4; ++i) { if (h->ev_up[i]) cudaEventDestroy(h->ev_up[i]); if (h->ev_run[i]) cudaEventDestroy(h->ev_run[i]); }
   if (h->h_meta) cudaFreeHost(h->h_meta);
   if (h->meta_done) cudaEventDestroy(h->meta_done);
   for (int i = 0; i <= FFPP_NUM_STAGES; ++i)

@@ -139,3 +139,17 @@ def test_full_size_configs_in_the_bench_launch_configuration(torch_cuda, ffpp_mo
     out2 = pp.run(torch_cuda.from_numpy(w.raw).cuda(), w.N_per_frame, w.frame_dims)
     torch_cuda.cuda.synchronize()
     compare(out2, ref, w)
+    if c >= 4:
+        # the host-buffer entry point at full size: config 5 (66 MB) is cut into four overlapped runs of whole frames
+        # (chunk starts on 16-byte raw offsets although 1280x720 frames are 8 bytes off), pageable and pinned outputs
+        compare(pp.run_host(w.raw, w.N_per_frame, w.frame_dims), ref, w)
+        torch = torch_cuda
+        out = ffpp_mod.Output()
+        out.density_offsets = pp.density_offsets(w.frame_dims)
+        out.boxes = torch.zeros((w.B, pp.top_k, 6), dtype=torch.float32).pin_memory()
+        out.counts = torch.zeros((w.B,), dtype=torch.int32).pin_memory()
+        out.density = torch.zeros((int(out.density_offsets[-1]),), dtype=torch.float32).pin_memory()
+        raw = torch.from_numpy(w.raw).pin_memory()
+        for _ in range(2):
+            pp.run_host(raw, w.N_per_frame, w.frame_dims, out=out)
+        compare(out, ref, w)
