@@ -877,10 +877,11 @@ __global__ void __launch_bounds__(K4_THREADS, 2) k4_resolve_emit(
   K4Misc* misc = reinterpret_cast<K4Misc*>(hist + K4_WARPS * 256);
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  // Which frame this CTA takes.  All CTAs start at once; the hardware hands out CTAs 0..S-1 one per SM and then CTA
-  // S+j to the SM of CTA j (checked with %smid), so with B < 2S frames the SMs of CTAs B-S..S-1 run ONE frame.  The
-  // frames are ranked by an estimate of their a4 time (edges, boxes, and the kept count the edge count implies); the
-  // 2S-B longest run alone, the next longest are paired with the shortest.
+  // Which frame this CTA takes.  All CTAs start at once; the hardware hands out CTAs 0..S-1 one per SM and doubles up
+  // after that (measured with %smid: the second CTA of an SM comes in a fixed order that only roughly follows the
+  // first, so which SMs stay single is approximate).  The frames are ranked by an estimate of their a4 time (edges,
+  // boxes, and the kept count the edge count implies): the 2S-B longest go to the CTAs expected to stay alone, the next
+  // longest are paired with the shortest.  What matters most is that long frames never pair with long ones.
   __shared__ int s_w[K4_MAXPERM];
   __shared__ int s_frame;
   {
