@@ -198,6 +198,38 @@ def test_every_radius_bucket_of_the_density_kernel(env, sigma, trunc, R):
     check(env, w)
 
 
+def test_non_finite_inputs_do_not_hang_and_agree_with_the_oracle(env):
+    """NaN logits never survive; non-finite distances must not hang or crash (their result is otherwise
+    unspecified).  Both sides happen to agree on them too: a box with a NaN/inf coordinate never suppresses and is
+    never suppressed (IoU is NaN or 0), and its centroid fails the in-frame test."""
+    torch, m, oracle_mod, gen = env
+    w = gen.make_config(2, B=2)
+    raw = w.raw.copy()
+    rng = np.random.default_rng(0)
+    js = rng.choice(8400, size=40, replace=False)
+    vals = [np.inf, -np.inf, np.nan, 60000.0, -60000.0]
+    for k, j in enumerate(js):
+        raw[j, k % 4] = vals[k % 5]
+        raw[j, 4] = 6.0 - 0.01 * k
+    raw[js[0] + 1, 4] = np.nan
+    raw[js[1] + 1, 4] = np.inf
+    pp = m.FFPP.for_workload(w)
+    out = pp.run(torch.from_numpy(raw).cuda(), w.N_per_frame, w.frame_dims)
+    torch.cuda.synchronize()
+    ref = oracle_mod.run(w.params, raw, w.N_per_frame, w.frame_dims)
+    assert np.array_equal(out.counts_numpy(), ref.counts)
+    g = out.boxes_numpy()
+    for f in range(2):
+        n = int(ref.counts[f])
+        assert np.array_equal(g[f, :n]["cand_index"], ref.boxes[f, :n]["cand_index"])
+        for k in ("x1", "y1", "x2", "y2"):
+            a, b = g[f, :n][k], ref.boxes[f, :n][k]
+            fin = np.isfinite(b)
+            assert np.array_equal(a[fin].view(np.uint32), b[fin].view(np.uint32)) and np.array_equal(np.isnan(a), np.isnan(b))
+    d = out.density_numpy()
+    assert np.isfinite(d).all() and np.all(np.abs(d - ref.density) <= np.maximum(1e-5, 1e-4 * np.abs(ref.density)))
+
+
 def test_abi_misuse_is_rejected(env):
     torch, m, oracle_mod, gen = env
     good = dict(max_frames=2, max_total_candidates=2 * 8400, max_frame_w=640, max_frame_h=640)
