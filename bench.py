@@ -4,7 +4,7 @@ post-processed frames/s and candidates/s at 1 B200; % of roofline per stage).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference]
 
-One "step" = one ffpp_run over one whole batch of the chosen config (all §8(a) rows a0-a6, five kernel
+One "step" = one ffpp_run over one whole batch of the chosen config (all §8(a) rows a0-a6, six kernel
 launches on one stream).  Default workload: config 5 (ragged 256-frame multi-zone batch, 6 639 360 candidates,
 66.4 MB fp16), the largest single-GPU configuration and the only one that exercises the ragged scheduler.
 Rank r of N generates its own batch (seed offset r): frames are independent, so N GPUs = N x the frames, no
@@ -402,7 +402,7 @@ def run_ours(args):
             "e2e": {"value": frames_all * e2e_steps / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": 1e3 * t_e2e / e2e_steps, "candidates_per_s": cand_all * e2e_steps / t_e2e,
                     "api": "ffpp_run_host (pinned host buffers, copies + sync inside the timed region)"},
-            "gpu_launches": 5 * K,
+            "gpu_launches": 6 * K,
             "warm_l2": {"ms_per_step": float(warm_ms.sum()), "frames_per_s": B / (float(warm_ms.sum()) * 1e-3),
                         "stages_ms": {nm: float(warm_ms[i]) for i, nm in enumerate(names)},
                         "a1_GB/s": alg_bytes["a1_threshold_compact"] / (float(warm_ms[1]) * 1e-3) / 1e9,

@@ -32,7 +32,7 @@ NUM_STAGES = 6
 STAGE_NAMES = ["a0_schedule", "a1_threshold_compact", "a2_sort_topk_decode", "a3_nms_mask", "a4_nms_sweep", "a5a6_density"]
 
 STAGE_KERNELS = {"a0_schedule": "host scheduler + memset", "a1_threshold_compact": "k1_threshold_compact",
-                 "a2_sort_topk_decode": "k2_select_bin", "a3_nms_mask": "k3_nms_edges", "a4_nms_sweep": "k4_resolve_emit",
+                 "a2_sort_topk_decode": "k2_select_bin", "a3_nms_mask": "k3_nms_edges", "a4_nms_sweep": "k4_resolve_order + k4e_emit",
                  "a5a6_density": "k5_density"}
 
 # fp32 instructions per IoU pair of the all-pairs bitmask method (4 min/max, 2 sub, 2 clamp, 1 mul, area

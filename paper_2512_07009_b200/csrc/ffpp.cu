@@ -60,6 +60,8 @@ struct ffpp_handle {
   float4* d_sp_sbox = nullptr;        // culling boxes
   void* d_sp_key = nullptr;
   uint8_t* d_hasin = nullptr;         // a3 -> a4: one byte per box, 1 = victim of at least one edge
+  void* d_kept_key = nullptr;         // a4: keys of the kept boxes in keep order, top_k per frame
+  uint16_t* d_kept_pos = nullptr;     // a4: their spatial positions
   uint8_t* d_k4_scratch = nullptr;    // a4 sort arrays of frames whose kept set does not fit shared memory
   uint16_t* d_cellstart = nullptr;    // kCellStride entries per frame: start position of every spatial cell
   uint32_t* d_edges = nullptr;
@@ -231,9 +233,16 @@ int launch_all(ffpp_handle* h, const void* raw, int B, cudaStream_t st, ffpp_box
   }
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[4], st));
   // a4 (+ a5 histogram)
-  k4_resolve_emit<KeyT><<<B, K4_THREADS, k4_smem_bytes((size_t)c.top_k, (size_t)c.kpad, sizeof(KeyT)), st>>>(
+  k4_resolve_order<KeyT><<<B, K4_THREADS, k4_smem_bytes((size_t)c.top_k, (size_t)c.kpad, sizeof(KeyT)), st>>>(
       frames, h->n_sorted(), h->d_sp_box, static_cast<const KeyT*>(h->d_sp_key), h->edge_ctr(), h->d_edges,
-      reinterpret_cast<const uint32_t*>(h->d_hasin), h->frame_err(), c, h->sm_count, h->d_k4_scratch, out_boxes, out_counts, h->d_hist32);
+      reinterpret_cast<const uint32_t*>(h->d_hasin), h->frame_err(), c, h->sm_count, h->d_k4_scratch,
+      static_cast<KeyT*>(h->d_kept_key), h->d_kept_pos, out_counts);
+  {
+    const dim3 g4e((unsigned)((h->max_nmax + K4E_THREADS - 1) / K4E_THREADS), (unsigned)B);
+    if (g4e.x > 0)
+      k4e_emit<KeyT><<<g4e, K4E_THREADS, 0, st>>>(frames, h->d_sp_box, static_cast<const KeyT*>(h->d_kept_key), h->d_kept_pos,
+                                                  out_counts, c, out_boxes, h->d_hist32);
+  }
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[5], st));
   // a6
   {
@@ -262,7 +271,7 @@ int set_kernel_attrs(ffpp_handle* h) {
   const size_t s2 = k2_smem_bytes((size_t)h->p.top_k, sizeof(KeyT));
   FFPP_CUDA(h, cudaFuncSetAttribute(k2_select_bin<kHalf, KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s2));
   const size_t s4 = k4_smem_bytes((size_t)h->p.top_k, (size_t)h->kpad, sizeof(KeyT));
-  FFPP_CUDA(h, cudaFuncSetAttribute(k4_resolve_emit<KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s4));
+  FFPP_CUDA(h, cudaFuncSetAttribute(k4_resolve_order<KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s4));
   return FFPP_OK;
 }
 
@@ -377,6 +386,8 @@ int ffpp_create(const ffpp_params* p, ffpp_handle** out) {
       (e = dalloc((void**)&h->d_sp_sbox, F * KP * sizeof(float4))) != cudaSuccess ||
       (e = dalloc(&h->d_sp_key, F * KP * (size_t)h->key_bytes)) != cudaSuccess ||
       (e = dalloc((void**)&h->d_hasin, F * KP)) != cudaSuccess ||
+      (e = dalloc(&h->d_kept_key, F * (size_t)p->top_k * (size_t)h->key_bytes)) != cudaSuccess ||
+      (e = dalloc((void**)&h->d_kept_pos, F * (size_t)p->top_k * sizeof(uint16_t))) != cudaSuccess ||
       (e = dalloc((void**)&h->d_k4_scratch, F * k4_scratch_bytes((size_t)p->top_k, (size_t)h->key_bytes))) != cudaSuccess ||
       (e = dalloc((void**)&h->d_cellstart, F * (size_t)kCellStride * sizeof(uint16_t))) != cudaSuccess ||
       (e = dalloc((void**)&h->d_edges, (size_t)h->edge_cap_total * sizeof(uint32_t))) != cudaSuccess ||
@@ -542,7 +553,7 @@ int ffpp_run_host(ffpp_handle* h, const void* raw, int32_t B, const int32_t* N_p
 int ffpp_destroy(ffpp_handle* h) {
   if (!h) return FFPP_OK;
   cudaFree(h->d_meta); cudaFree(h->d_surv_keys); cudaFree(h->d_counters); cudaFree(h->d_sel_box); cudaFree(h->d_sp_box);
-  cudaFree(h->d_sp_sbox); cudaFree(h->d_sp_key); cudaFree(h->d_cellstart); cudaFree(h->d_hasin); cudaFree(h->d_k4_scratch); cudaFree(h->d_edges);
+  cudaFree(h->d_sp_sbox); cudaFree(h->d_sp_key); cudaFree(h->d_cellstart); cudaFree(h->d_hasin); cudaFree(h->d_k4_scratch); cudaFree(h->d_kept_key); cudaFree(h->d_kept_pos); cudaFree(h->d_edges);
   cudaFree(h->d_hist32);
   cudaFree(h->d_in); cudaFree(h->d_out_boxes); cudaFree(h->d_out_counts); cudaFree(h->d_out_density);
   if (h->s_h2d) cudaStreamDestroy(h->s_h2d);

@@ -654,7 +654,7 @@ __global__ void __launch_bounds__(K3_THREADS) k3_nms_edges(const FrameDesc* __re
 }
 
 // =====================================================================================================
-// a4 — greedy resolve + order + output gather + centroid histogram (north_star (c) second half; SURVEY §8(a) a4-a5,
+// a4 — greedy resolve + order (+ k4e_emit: output gather + centroid histogram) (north_star (c) second half; SURVEY §8(a) a4-a5,
 // §8(c) O5-O7).  One 512-thread CTA per frame, two CTAs per SM (296 slots: a 256-frame batch is resident at once and
 // the barriers of one frame are hidden behind the work of another).
 // Greedy NMS in the order of O4 is the unique solution of
@@ -671,10 +671,9 @@ __global__ void __launch_bounds__(K3_THREADS) k3_nms_edges(const FrameDesc* __re
 // reads it eight edges at a time (the list lives in L2: memory-level parallelism, not latency, must pace the loop)
 // and compacts it in place, so a round only re-reads the edges that are still undecided.
 // Then the kept boxes are ordered: their keys and spatial positions are gathered through a prefix sum of the kept
-// bitmap and sorted by key with a bitonic network (this is where the (score desc, index asc) order of O4 is
-// materialised — on the kept set only); output row r is the r-th pair, written with its sigmoid score and
-// candidate index, and its centroid is binned into the frame's histogram (a5).  The sort arrays live in shared
-// memory when the kept count (rounded up to a power of two) fits, else in a global scratch area.
+// bitmap and sorted by key (bitonic network up to 1024, LSD radix beyond; this is where the (score desc, index asc)
+// order of O4 is materialised — on the kept set only) and the ordered (key, position) list goes to global memory for
+// the flat emit kernel k4e_emit.  The sort arrays live in shared memory when they fit, else in a global scratch area.
 // =====================================================================================================
 constexpr int K4_THREADS = 512;
 constexpr int K4_WARPS = K4_THREADS / 32;
@@ -856,11 +855,11 @@ __device__ __forceinline__ void k4_bitonic(KeyT* kA, uint16_t* pA, KeyT* kB, uin
 }
 
 template <typename KeyT>
-__global__ void __launch_bounds__(K4_THREADS, 2) k4_resolve_emit(
+__global__ void __launch_bounds__(K4_THREADS, 2) k4_resolve_order(
     const FrameDesc* __restrict__ frames, const int* __restrict__ n_sorted, const float4* __restrict__ sp_box,
     const KeyT* __restrict__ sp_key, const int* __restrict__ edge_ctr, uint32_t* edges,
     const uint32_t* __restrict__ hasin, const int* __restrict__ frame_err, Consts cst, int sm_count, uint8_t* __restrict__ scratch,
-    ffpp_box* __restrict__ out_boxes, int* __restrict__ out_counts, uint32_t* __restrict__ hist32) {
+    KeyT* __restrict__ kept_key, uint16_t* __restrict__ kept_pos, int* __restrict__ out_counts) {
   extern __shared__ __align__(16) uint8_t smem[];
   __shared__ FrameDesc fd;
   const int K = cst.top_k, kpad = cst.kpad;
@@ -1053,26 +1052,36 @@ __global__ void __launch_bounds__(K4_THREADS, 2) k4_resolve_emit(
   }
   FFPP_PHASE(f, 5);
 
-  // ---- emit: output row r = r-th kept box in key order ----
-  for (int r0 = tid; r0 < m; r0 += 4 * K4_THREADS) {
-    KeyT key[4];
-    float4 bx[4];
-#pragma unroll
-    for (int u = 0; u < 4; ++u) {
-      const int r = r0 + u * K4_THREADS;
-      if (r < m) { key[u] = kk[r]; bx[u] = sp_box[obase + pp[r]]; }
-    }
-#pragma unroll
-    for (int u = 0; u < 4; ++u) {
-      const int r = r0 + u * K4_THREADS;
-      if (r < m) emit_kept(fd, cst, out_boxes + (int64_t)f * K + r, bx[u], logit_of_key<KeyT>(key[u]), idx_of_key<KeyT>(key[u]), hist32);
-    }
+  // ---- hand the ordered kept list (key, spatial position) to the flat emit kernel: writing 369 k detections is
+  // per-box work with no per-frame structure, and on one SM it was a third of a long frame's a4 time ----
+  {
+    KeyT* ok = kept_key + (int64_t)f * K;
+    uint16_t* op = kept_pos + (int64_t)f * K;
+    for (int r = tid; r < m; r += K4_THREADS) { ok[r] = kk[r]; op[r] = pp[r]; }
   }
 #ifdef FFPP_PROFILE_PHASES
   __syncthreads();
   FFPP_PHASE(f, 6);
   if (tid == 0) g_phase[f][7] = ((unsigned long long)n << 40) | ((unsigned long long)E << 16) | (unsigned long long)m;
 #endif
+}
+
+// a4, second launch — FLAT emit over (frame, output row): row r of frame f is the r-th entry of the ordered kept list;
+// the detection is written with its sigmoid score and candidate index (O6) and its centroid is binned into the
+// frame's histogram (a5, O7 first half).
+constexpr int K4E_THREADS = 256;
+template <typename KeyT>
+__global__ void __launch_bounds__(K4E_THREADS) k4e_emit(const FrameDesc* __restrict__ frames, const float4* __restrict__ sp_box,
+                                                        const KeyT* __restrict__ kept_key, const uint16_t* __restrict__ kept_pos,
+                                                        const int* __restrict__ out_counts, Consts cst,
+                                                        ffpp_box* __restrict__ out_boxes, uint32_t* __restrict__ hist32) {
+  const int f = blockIdx.y;
+  const int r = blockIdx.x * K4E_THREADS + threadIdx.x;
+  if (r >= out_counts[f]) return;                               // also frames flagged -1
+  const int64_t o = (int64_t)f * cst.top_k + r;
+  const KeyT key = kept_key[o];
+  const float4 bx = sp_box[(int64_t)f * cst.kpad + kept_pos[o]];
+  emit_kept(frames[f], cst, out_boxes + o, bx, logit_of_key<KeyT>(key), idx_of_key<KeyT>(key), hist32);
 }
 
 // =====================================================================================================
