@@ -260,14 +260,11 @@ int32_t oracle_run(const oracle_params* p, const void* raw, int32_t B, const int
     if (sorted_counts) sorted_counts[f] = (int32_t)sv.size();
     if (sorted_idx)
       for (int32_t k = 0; k < p->top_k; ++k) sorted_idx[(int64_t)f * p->top_k + k] = k < (int32_t)sv.size() ? sv[(size_t)k].idx : -1;
-    // O5: greedy NMS against earlier kept boxes
-    std::vector<int32_t> kept;
-    for (size_t i = 0; i < sv.size(); ++i) {
-      bool keep = true;
-      for (size_t k = 0; k < kept.size() && keep; ++k)
-        if (iou(sv[(size_t)kept[k]].box, sv[i].box) > p->iou_thresh) keep = false;
-      if (keep) kept.push_back((int32_t)i);
-    }
+    // O5: greedy NMS against earlier kept boxes — the same routine the 50-box brute-force pin exercises
+    std::vector<float> sb(sv.size() * 4);
+    for (size_t i = 0; i < sv.size(); ++i) std::memcpy(&sb[i * 4], sv[i].box, 16);
+    std::vector<int32_t> kept(sv.size() + 1);
+    kept.resize((size_t)oracle_nms_sorted(sb.data(), (int32_t)sv.size(), p->iou_thresh, kept.data()));
     // O6: outputs; reported score = sigmoid(z) in fp32 (A8)
     std::vector<float> kb(kept.size() * 4);
     for (size_t k = 0; k < kept.size(); ++k) {
