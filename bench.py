@@ -4,24 +4,29 @@ post-processed frames/s and candidates/s at 1 B200; % of roofline per stage).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference]
 
-One "step" = one ffpp_run over one whole batch of the chosen config (all §8(a) rows a0-a6, six kernel
-launches on one stream).  Default workload: config 5 (ragged 256-frame multi-zone batch, 6 639 360 candidates,
-66.4 MB fp16), the largest single-GPU configuration and the only one that exercises the ragged scheduler.
+One "step" = one ffpp_run over one whole batch of the chosen config (all §8(a) rows a0-a6: seven kernel launches
+and one counter memset on one stream).  Default workload: config 5 (ragged 256-frame multi-zone batch, 6 639 360
+candidates, 66.4 MB fp16), the largest single-GPU configuration and the only one that exercises the ragged
+scheduler; the default single-GPU run also measures configs 1-4 briefly and carries them in `configs`.
 Rank r of N generates its own batch (seed offset r): frames are independent, so N GPUs = N x the frames, no
-data-path collective ("scaling": "weak").
+data-path collective ("scaling": "weak").  `--gpus N` without a torchrun environment re-executes itself under
+`python -m torch.distributed.run --nproc-per-node N`.
 
-Timing: every timed step is bracketed by CUDA events on the launching stream; L2 (126 MB) is flushed between
-steps by writing a 512 MB scratch buffer outside the event pair; the K step times are summed, the sum is
-max-reduced over ranks, and the whole timed loop sits between barrier + torch.cuda.synchronize() on both sides.
-`e2e` is the same metric through ffpp_run_host with pinned HOST buffers (H2D of the raw head output and D2H of
-counts, density and kept boxes inside the timed region).  `--impl reference` times the CPU oracle (oracle/) on
-a bounded sample; it is the only place besides `cpu_baseline` where bench.py executes oracle/.
+Timing: every timed step is bracketed by CUDA events on the launching stream.  Between steps L2 (126 MB) is left
+COLD AND CLEAN: a 512 MB write evicts everything, then a 512 MB read (k0_stream_read) replaces the dirty lines of
+that write with clean ones, so the step's first kernel does not compete with write-back traffic; both happen
+outside the event pair.  The K step times are summed, the sum is max-reduced over ranks, and the timed loop sits
+between barrier + torch.cuda.synchronize() on both sides.  `e2e` is the same metric through ffpp_run_host with
+pinned HOST buffers (H2D of the raw head output and D2H of counts, density and kept boxes inside the timed
+region).  `--impl reference` times the CPU oracle (oracle/) on a bounded sample; it is the only place besides
+`cpu_baseline` where bench.py executes oracle/.
 """
 from __future__ import annotations
 
 import argparse
 import json
 import os
+import socket
 import subprocess
 import sys
 import threading
@@ -43,6 +48,13 @@ CONFIG_DESC = {
     4: "config4: B=64 1920x1088 fp16 [64,42840,5]",
     5: "config5: ragged B=256 (64 each 640x640/1280x1280/1920x1088/1280x720, interleaved) fp16, 6639360 candidates",
 }
+
+# fp32 lane-instructions of the a3 method's own work (DESIGN.md §6 a3): a culling-box test is four
+# compares, an exact IoU is 15 fp32 instructions (4 min/max, 2 sub, 2 clamp, 1 mul, 2 area mul, 2 area sub, add, sub,
+# multiply-or-divide + compare)
+A3_OPS_PER_CULL_TEST = 4
+A3_OPS_PER_EXACT_IOU = 15
+FP32_LANES_PER_SM = 128
 
 
 def load_peaks():
@@ -114,6 +126,19 @@ def pair_count(n_sorted: np.ndarray) -> int:
     return int((n * (n - 1) // 2).sum())
 
 
+def free_port() -> int:
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def respawn_under_torchrun(args) -> int:
+    """`python bench.py --gpus N` outside a torchrun environment: start the N ranks ourselves (one process per GPU)."""
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(free_port()), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd, cwd=ROOT)
+
+
 # --------------------------------------------------------------------------------------------------------------
 # reference arm: the oracle as it stands, on the host cores
 # --------------------------------------------------------------------------------------------------------------
@@ -154,9 +179,9 @@ def run_reference(args):
     fps = nf * args.steps / t
     sample = f"first {nf} of {w.B} frames of {w.name} per step ({rows} candidates), single thread"
     line = {
-        "impl": "reference", "metric": METRIC, "value": fps, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "impl": "reference", "metric": METRIC, "value": fps, "unit": UNIT, "n_gpus": max(args.gpus, world), "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "vs_baseline": None, "dtype": "f32", "input_dtype": w.params["dtype"], "data": "synthetic",
         "config": {"workload": CONFIG_DESC[args.config], "sample": sample},
         "candidates_per_s": rows * args.steps / t,
         "cpu_baseline": {"value": fps, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
@@ -181,13 +206,137 @@ def reduce_over_ranks(total_ms: float, t_e2e: float, frames: float, cands: float
     return float(t[0]), float(t[1]), float(u[0]), float(u[1])
 
 
+def a3_roofline(work: np.ndarray, ms: float, sm_count: int, sm_mhz: float) -> dict:
+    """Method's own fp32 lane-instructions of one a3 launch (device-counted) against the fp32 lane peak."""
+    ops = A3_OPS_PER_CULL_TEST * int(work[0]) + A3_OPS_PER_EXACT_IOU * int(work[1])
+    peak = sm_count * FP32_LANES_PER_SM * sm_mhz * 1e6
+    ach = ops / (ms * 1e-3)
+    return {"bound": "alu", "achieved": ach / 1e12, "peak": peak / 1e12, "unit": "T fp32 lane-instr/s", "frac": ach / peak,
+            "counted_work": {"culling_box_tests": int(work[0]), "exact_ious": int(work[1]), "edges": int(work[2]),
+                             "frames_on_overflow_path": int(work[3]), "lane_instructions": ops,
+                             "how": "device counters of the counting instantiation of the a3 kernel, separate untimed run "
+                                    f"(ffpp_debug_count_work); {A3_OPS_PER_CULL_TEST} per culling test + {A3_OPS_PER_EXACT_IOU} per exact IoU"},
+            "peak_source": f"{sm_count} SM x {FP32_LANES_PER_SM} fp32 lanes x {sm_mhz:.0f} MHz (sm_count from the handle, clocks.max.sm)"}
+
+
+# --------------------------------------------------------------------------------------------------------------
+# one config on this rank's GPU
+# --------------------------------------------------------------------------------------------------------------
+class Bench:
+    def __init__(self, c: int, rank: int, flush, stream):
+        import torch
+        import flockgen
+        import paper_2512_07009_b200 as ffpp
+        self.torch, self.ffpp = torch, ffpp
+        self.c = c
+        self.w = flockgen.make_config(c, seed_offset=rank)
+        self.pp = ffpp.FFPP.for_workload(self.w)
+        self.info = self.pp.info()
+        self.stream = stream
+        self.flush = flush
+        self.raw_pinned = torch.from_numpy(self.w.raw).pin_memory()
+        self.raw_dev = self.raw_pinned.cuda(non_blocking=False)
+        self.out = self.pp.alloc_outputs(self.w.B, self.w.frame_dims)
+
+    def step(self):
+        self.pp.run(self.raw_dev, self.w.N_per_frame, self.w.frame_dims, out=self.out, stream=self.stream)
+
+    def flush_l2(self, clean: bool = True):
+        """Outside every event pair.  512 MB write evicts the whole L2; the 512 MB read that follows replaces the dirty
+        lines of that write with clean ones (cold AND clean: nothing is being written back while the step runs)."""
+        self.flush.zero_()
+        if clean:
+            self.pp.stream_read(self.flush, self.stream)
+
+    def timed_steps(self, steps: int, clean: bool = True) -> np.ndarray:
+        torch = self.torch
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        for k in range(steps):
+            self.flush_l2(clean)
+            ev[k][0].record(self.stream)
+            self.step()
+            ev[k][1].record(self.stream)
+        torch.cuda.synchronize()
+        return np.array([a.elapsed_time(b) for a, b in ev], dtype=np.float64)
+
+    def stage_ms(self, iters: int, mode: str) -> np.ndarray:
+        """Per-stage durations from the library's own events on the launching stream.  mode: cold_clean | cold_dirty | warm."""
+        torch = self.torch
+        self.pp.set_stage_timing(True)
+        acc = []
+        for i in range(iters + (2 if mode == "warm" else 0)):
+            if mode != "warm":
+                self.flush_l2(mode == "cold_clean")
+            self.step()
+            torch.cuda.synchronize()
+            acc.append(self.pp.stage_ms().astype(np.float64))
+        self.pp.set_stage_timing(False)
+        return np.mean(np.stack(acc[2:] if mode == "warm" else acc), axis=0)
+
+    def read_floor_ms(self, clean: bool) -> float:
+        torch = self.torch
+        rd = []
+        for _ in range(8):
+            self.flush_l2(clean)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(self.stream); self.pp.stream_read(self.raw_dev, self.stream); e1.record(self.stream)
+            torch.cuda.synchronize()
+            rd.append(e0.elapsed_time(e1))
+        return float(np.median(rd[2:]))
+
+    def counted_work(self) -> np.ndarray:
+        self.pp.count_work(True)
+        self.step()
+        self.torch.cuda.synchronize()
+        work = self.pp.debug_read(4, self.w.B)
+        self.pp.count_work(False)
+        self.step()
+        self.torch.cuda.synchronize()
+        return work
+
+    def alg_bytes(self, n_surv, n_sorted, kept):
+        w = self.w
+        elem = 2 if w.params["dtype"] == "fp16" else 4
+        key_b = self.info.key_bits // 8
+        row_b = 5 * elem
+        cells = int(self.out.density_offsets[-1])
+        n_sv, n_in, kept_n = int(n_surv.sum()), int(n_sorted.sum()), int(kept.sum())
+        return {
+            "a1_threshold_compact": w.total_candidates * row_b + n_sv * key_b,   # read every row once, write one key per survivor
+            "a2_select_decode_bin": n_sv * key_b + n_in * (row_b + 36),          # read keys, gather top-K rows, write box + culling box + key
+            "a4_nms_resolve_emit": n_in * 24 + kept_n * 24 + 4 * w.B,            # read top-K records, write kept records + counts
+            "a5a6_density": 4 * cells + 2 * cells + 16 * kept_n,                # histogram read, every density cell written once, kept boxes read
+        }, row_b, cells
+
+
+def quick_config(c: int, rank: int, flush, stream, hbm_peak: float) -> dict:
+    """Configs other than the main one: a short cold-clean measurement for the `configs` block."""
+    b = Bench(c, rank, flush, stream)
+    for _ in range(3):
+        b.flush_l2(); b.step()
+    b.torch.cuda.synchronize()
+    B = b.w.B
+    n_sorted, n_surv = b.pp.debug_read(1, B), b.pp.debug_read(0, B)
+    kept = b.out.counts_numpy().astype(np.int64)
+    step_ms = b.timed_steps(10)
+    st = b.stage_ms(5, "cold_clean")
+    ab, _, _ = b.alg_bytes(n_surv, n_sorted, kept)
+    ms = float(np.mean(step_ms))
+    res = {"workload": CONFIG_DESC[c], "ms_per_step": ms, "frames_per_s": B / (ms * 1e-3), "candidates_per_s": b.w.total_candidates / (ms * 1e-3),
+           "a1_frac_of_hbm_peak": ab["a1_threshold_compact"] / (st[1] * 1e-3) / 1e9 / hbm_peak,
+           "a6_frac_of_hbm_peak": ab["a5a6_density"] / (st[5] * 1e-3) / 1e9 / hbm_peak,
+           "stages_ms": {nm: float(st[i]) for i, nm in enumerate(b.ffpp.STAGE_NAMES)}, "steps": 10,
+           "kept": int(kept.sum()), "entering_nms": int(n_sorted.sum())}
+    b.pp.close()
+    return res
+
+
 # --------------------------------------------------------------------------------------------------------------
 # our arm
 # --------------------------------------------------------------------------------------------------------------
 def run_ours(args):
     import torch
     import torch.distributed as dist
-    import flockgen
     import paper_2512_07009_b200 as ffpp
 
     rank, local_rank, world = dist_env()
@@ -199,77 +348,45 @@ def run_ours(args):
     hbm_peak, peak_src, sm_max_mhz = load_peaks()
 
     c = args.config
-    w = flockgen.make_config(c, seed_offset=rank)
-    B, total_cand = w.B, w.total_candidates
-    pp = ffpp.FFPP.for_workload(w)
-    info = pp.info()
     stream = torch.cuda.current_stream()
-    raw_pinned = torch.from_numpy(w.raw).pin_memory()
-    raw_dev = raw_pinned.cuda(non_blocking=False)
-    out = pp.alloc_outputs(B, w.frame_dims)
     flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
+    b = Bench(c, rank, flush, stream)
+    w, pp, info, out = b.w, b.pp, b.info, b.out
+    B, total_cand = w.B, w.total_candidates
+    sm_count = int(info.sm_count)
 
     def barrier():
         if world > 1:
             dist.barrier()
 
-    def step_device():
-        pp.run(raw_dev, w.N_per_frame, w.frame_dims, out=out, stream=stream)
-
     # ---- warm-up ----
-    for _ in range(max(args.warmup, 3)):
-        flush.zero_()
-        step_device()
+    W = max(args.warmup, 3)
+    for _ in range(W):
+        b.flush_l2(); b.step()
     torch.cuda.synchronize()
     n_sorted = pp.debug_read(1, B)
     n_surv = pp.debug_read(0, B)
     kept = out.counts_numpy().astype(np.int64)
     pairs = pair_count(n_sorted)
 
-    # ---- timed: device-resident inputs ----
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    # ---- timed: device-resident inputs, cold and clean L2 ----
     sampler = ClockSampler(local_rank)
     barrier(); torch.cuda.synchronize()
     sampler.start()
     t_wall0 = time.perf_counter()
-    for k in range(args.steps):
-        flush.zero_()
-        ev[k][0].record(stream)
-        step_device()
-        ev[k][1].record(stream)
+    step_ms = b.timed_steps(args.steps)
     torch.cuda.synchronize(); barrier()
     t_wall = time.perf_counter() - t_wall0
-    step_ms = np.array([a.elapsed_time(b) for a, b in ev], dtype=np.float64)
     total_ms = float(step_ms.sum())
 
-    # ---- per-stage durations (library's own events on the launching stream), cold L2, same launch configuration ----
-    pp.set_stage_timing(True)
-    stage = []
-    for _ in range(min(max(args.steps, 3), 20)):
-        flush.zero_()
-        step_device()
-        torch.cuda.synchronize()
-        stage.append(pp.stage_ms().astype(np.float64))
-    stage_ms = np.mean(np.stack(stage), axis=0)
-    # ---- the same, WARM: no flush, the raw head output (if it fits) still in the 126 MB L2 as it would be right after
-    # the detector wrote it (SURVEY §8(d) asks for both regimes); reported beside the cold numbers, never instead ----
-    warm = []
-    for _ in range(min(max(args.steps, 3), 20) + 2):
-        step_device()
-        torch.cuda.synchronize()
-        warm.append(pp.stage_ms().astype(np.float64))
-    pp.set_stage_timing(False)
-    warm_ms = np.mean(np.stack(warm[2:]), axis=0)
-
-    # ---- calibration: a plain read of the same raw buffer, same cold-L2 regime, CUDA events on the same stream ----
-    rd = []
-    for _ in range(8):
-        flush.zero_()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(stream); pp.stream_read(raw_dev, stream); e1.record(stream)
-        torch.cuda.synchronize()
-        rd.append(e0.elapsed_time(e1))
-    read_floor_ms = float(np.median(rd[2:]))
+    # ---- per-stage durations (library's own events on the launching stream), same launch configuration ----
+    n_it = min(max(args.steps, 3), 20)
+    stage_ms = b.stage_ms(n_it, "cold_clean")
+    dirty_ms = b.stage_ms(n_it, "cold_dirty")
+    warm_ms = b.stage_ms(n_it, "warm")
+    read_clean_ms = b.read_floor_ms(True)
+    read_dirty_ms = b.read_floor_ms(False)
+    work = b.counted_work()                 # separate, untimed: the counting instantiation of the a3 kernel
 
     # ---- e2e: host buffers through ffpp_run_host ----
     cells = int(out.density_offsets[-1])
@@ -280,7 +397,7 @@ def run_ours(args):
     hout.boxes, hout.counts, hout.density, hout.density_offsets = h_boxes, h_counts, h_density, out.density_offsets
 
     def step_host():
-        pp.run_host(raw_pinned, w.N_per_frame, w.frame_dims, out=hout, stream=stream)
+        pp.run_host(b.raw_pinned, w.N_per_frame, w.frame_dims, out=hout, stream=stream)
 
     e2e_steps = args.steps
     for _ in range(3):
@@ -288,7 +405,7 @@ def run_ours(args):
     barrier(); torch.cuda.synchronize()
     t_e2e = 0.0
     for _ in range(e2e_steps):
-        flush.zero_(); torch.cuda.synchronize()
+        b.flush_l2(); torch.cuda.synchronize()
         t0 = time.perf_counter()
         step_host()
         t_e2e += time.perf_counter() - t0
@@ -296,6 +413,27 @@ def run_ours(args):
     clocks = sampler.stop()
     h2d = int(w.raw.nbytes)
     d2h = int(4 * B + 4 * cells + 24 * int(kept.sum()))
+    # PCIe floor of the same transfers: pinned H2D of the raw buffer and pinned D2H of the density, each alone
+    def copy_ms(dst, src):
+        ts = []
+        for _ in range(5):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream); dst.copy_(src, non_blocking=True); e1.record(stream)
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        return float(np.median(ts[1:]))
+    h2d_ms = copy_ms(b.raw_dev, b.raw_pinned)
+    d2h_ms = copy_ms(h_density, out.density) * (d2h / max(4 * cells, 1))
+
+    # ---- the other configs (single-GPU default run only): short cold-clean measurements ----
+    configs = {}
+    if world == 1 and not args.no_other_configs:
+        for cc in (1, 2, 3, 4, 5):
+            if cc != c:
+                try:
+                    configs[str(cc)] = quick_config(cc, rank, flush, stream, hbm_peak)
+                except Exception as exc:           # reported, never fatal for the main line
+                    configs[str(cc)] = {"workload": CONFIG_DESC[cc], "error": str(exc)}
 
     # ---- reduce over ranks ----
     total_ms, t_e2e, frames_all, cand_all = reduce_over_ranks(total_ms, t_e2e, float(B), float(total_cand), world, "cuda")
@@ -304,73 +442,56 @@ def run_ours(args):
         K = args.steps
         fps = frames_all * K / (total_ms * 1e-3)
         cps = cand_all * K / (total_ms * 1e-3)
-        elem = 2 if w.params["dtype"] == "fp16" else 4
-        key_b = info.key_bits // 8
-        cell_b = 4 * cells
         kept_n = int(kept.sum())
-        # algorithmic bytes / ops per launch (DESIGN.md §6 "Kernels and rooflines")
-        row_b = 5 * elem
-        n_sv, n_in = int(n_surv.sum()), int(n_sorted.sum())
-        alg_bytes = {
-            "a1_threshold_compact": total_cand * row_b + n_sv * key_b,           # read every row once, write one key per survivor
-            "a2_sort_topk_decode": n_sv * key_b + n_in * (row_b + 24),            # read keys, gather top-K rows, write box+logit+index
-            "a4_nms_sweep": n_in * 24 + kept_n * 24 + 4 * B,                      # read sorted records, write kept records + counts
-            "a5a6_density": cell_b + 16 * kept_n,                                 # read kept boxes, write every density cell once
-        }
+        alg_bytes, row_b, _ = b.alg_bytes(n_surv, n_sorted, kept)
+        cell_b = 4 * cells
         stages = {}
         names = ffpp.STAGE_NAMES
         for i, nm in enumerate(names):
-            stages[nm] = {"ms": float(stage_ms[i]), "share_of_step": float(stage_ms[i] / stage_ms.sum())}
+            stages[nm] = {"ms": float(stage_ms[i]), "share_of_step": float(stage_ms[i] / stage_ms.sum()), "kernels": ffpp.STAGE_KERNELS[nm],
+                          "ms_cold_dirty": float(dirty_ms[i]), "ms_warm": float(warm_ms[i])}
             if nm in alg_bytes:
                 gbs = alg_bytes[nm] / (stage_ms[i] * 1e-3) / 1e9
                 stages[nm].update({"algorithmic_bytes": alg_bytes[nm], "GB/s": gbs, "frac_of_hbm_peak": gbs / hbm_peak})
         s1 = stages["a1_threshold_compact"]
-        s1["plain_read_of_same_bytes"] = {"ms": read_floor_ms, "GB/s": total_cand * row_b / (read_floor_ms * 1e-3) / 1e9,
-                                          "frac_of_hbm_peak": total_cand * row_b / (read_floor_ms * 1e-3) / 1e9 / hbm_peak,
-                                          "note": "k0_stream_read over the raw head output, cold L2 after the same 512 MB write "
-                                                  "flush: what a pure read of this many bytes reaches on this GPU"}
-        s1["frac_of_plain_read"] = read_floor_ms / float(stage_ms[1])
-        s3 = stages["a3_nms_mask"]; s3["iou_pairs"] = pairs
-        s3["Gpairs/s"] = pairs / (stage_ms[3] * 1e-3) / 1e9
-        # a3 ALU ceiling of the all-pairs method: 148 SM x 128 fp32 lanes x clock / 15 instr per IoU pair
-        alu_peak_gpairs = 148 * 128 * sm_max_mhz * 1e6 / ffpp.NMS_ALU_OPS_PER_PAIR / 1e9
-        s3["frac_of_allpairs_alu_peak"] = s3["Gpairs/s"] / alu_peak_gpairs
+        raw_bytes = total_cand * row_b
+        s1["plain_read_of_same_bytes"] = {
+            "ms": read_clean_ms, "GB/s": raw_bytes / (read_clean_ms * 1e-3) / 1e9, "frac_of_hbm_peak": raw_bytes / (read_clean_ms * 1e-3) / 1e9 / hbm_peak,
+            "ms_cold_dirty": read_dirty_ms,
+            "note": "k0_stream_read over the raw head output under the same cold-clean regime: what a pure read of this many bytes reaches"}
+        s1["frac_of_plain_read"] = read_clean_ms / float(stage_ms[1])
+        s3 = stages["a3_nms_pairs"]
+        s3["iou_pairs_decided"] = pairs
+        s3["Gpairs/s_decided"] = pairs / (stage_ms[3] * 1e-3) / 1e9
+        r3 = a3_roofline(work, float(stage_ms[3]), sm_count, sm_max_mhz)
+        # speed-up over the all-pairs bitmask method at ITS ALU ceiling (context, not a roofline fraction)
+        allpairs_ceiling = sm_count * FP32_LANES_PER_SM * sm_max_mhz * 1e6 / A3_OPS_PER_EXACT_IOU
+        s3["dense_equiv_speedup"] = (pairs / (stage_ms[3] * 1e-3)) / allpairs_ceiling
+        s3["alu"] = {k: r3[k] for k in ("achieved", "peak", "unit", "frac", "counted_work")}
         # dominant kernel = the stage with the largest share of the step
         dom = int(np.argmax(stage_ms[1:])) + 1
         if dom == 3:
-            roofline = {"kernel": ffpp.STAGE_KERNELS[names[dom]], "bound": "alu", "achieved": s3["Gpairs/s"], "peak": alu_peak_gpairs,
-                        "unit": "Gpair/s", "frac": s3["Gpairs/s"] / alu_peak_gpairs, "traffic": None,
-                        "peak_source": f"148 SM x 128 fp32 lanes x {sm_max_mhz:.0f} MHz / {ffpp.NMS_ALU_OPS_PER_PAIR} fp32 instr per IoU pair "
-                                       "(SURVEY §8(d) all-pairs ceiling; DESIGN.md §6 a3)",
-                        "note": "pairs = full upper triangle n'(n'-1)/2 per frame that the launch DECIDES; the spatially tiled kernel "
-                                "decides most of them by bounding-box culling without evaluating them, so frac > 1 is possible and "
-                                "means 'faster than the all-pairs method can go', not 'above the hardware'"}
+            roofline = dict(r3)
+            roofline["dense_equiv_speedup"] = s3["dense_equiv_speedup"]
         else:
             sd = stages[names[dom]]
-            roofline = {"kernel": ffpp.STAGE_KERNELS[names[dom]], "bound": "hbm", "achieved": sd["GB/s"], "peak": hbm_peak, "unit": "GB/s",
-                        "frac": sd["GB/s"] / hbm_peak, "traffic": None, "peak_source": peak_src}
+            roofline = {"bound": "hbm", "achieved": sd["GB/s"], "peak": hbm_peak, "unit": "GB/s", "frac": sd["GB/s"] / hbm_peak, "peak_source": peak_src}
+        roofline["kernel"] = ffpp.STAGE_KERNELS[names[dom]]
         roofline["stage"] = names[dom]
         roofline["avg_launch_ms"] = float(stage_ms[dom])
-        roofline["hbm_peak_source"] = peak_src
-        tr_path = os.path.join(ROOT, "profiles", f"traffic_config{c}.csv")
-        if os.path.exists(tr_path):      # per-launch numbers of the committed ncu --set full capture of this config
+        roofline["traffic"] = None
+        tr_path = os.path.join(ROOT, "profiles", f"r2_traffic_config{c}.csv")
+        if os.path.exists(tr_path):      # STATIC: per-launch numbers of the committed ncu --set full capture of this config
             import csv
             with open(tr_path, newline="") as fh:
                 rows = {r["kernel"]: r for r in csv.DictReader(fh)}
-            k = rows.get(roofline["kernel"])
+            k = rows.get(roofline["kernel"].split(" ")[0])
             if k:
                 k = {kk: float(vv) for kk, vv in k.items() if kk != "kernel"}
-            tr = {"source": "profiles/r1_v4_config5_config4_ncu.md (ncu --set full, one launch of each kernel, cold cache)"}
-            if k:
                 roofline["traffic"] = k["dram_bytes"]            # dram__bytes_read.sum + dram__bytes_write.sum
-                roofline["traffic_source"] = tr.get("source")
-                # issue-slot view of the same launch: warp instructions of the capture over the LIVE duration,
-                # against 4 schedulers x 1 warp instruction per clock per SM
-                issue_peak = 148 * 4 * sm_max_mhz * 1e6
-                roofline["issue"] = {"warp_instructions": k["warp_instructions"],
-                                     "achieved_Ginst_s": k["warp_instructions"] / (float(stage_ms[dom]) * 1e-3) / 1e9,
-                                     "peak_Ginst_s": issue_peak / 1e9,
-                                     "frac": k["warp_instructions"] / (float(stage_ms[dom]) * 1e-3) / issue_peak}
+                roofline["static_from_ncu_capture"] = {
+                    "source": f"profiles/r2_traffic_config{c}.csv (one ncu --set full launch of the committed build; NOT measured by this run)",
+                    **{kk: k[kk] for kk in k if kk != "dram_bytes"}}
         # whole step against HBM: bytes the path must move (raw in, three outputs out) / device step time
         step_bytes = total_cand * row_b + 24 * kept_n + 4 * B + cell_b
         step_gbs = step_bytes / (float(np.median(step_ms)) * 1e-3) / 1e9
@@ -379,38 +500,48 @@ def run_ours(args):
                          "over the median device step time of this rank; every intermediate is overhead against this bound"}
 
         # ---- CPU baseline: the oracle as it stands on this box's host cores, bounded sample ----
-        cpu = None
-        if world == 1 or True:
-            try:
-                t_cpu, nf, rows = oracle_time(w, CPU_BASELINE_FRAMES[c])
-                cpu = {"value": nf / t_cpu, "unit": UNIT, "cores": 1, "kind": "oracle",
-                       "sample": f"first {nf} of {B} frames of {w.name} ({rows} candidates), one pass, single thread, {t_cpu:.2f} s",
-                       "candidates_per_s": rows / t_cpu, "host_cpus": os.cpu_count()}
-            except Exception as exc:  # the baseline is reported, never required for the GPU numbers
-                cpu = {"value": None, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": f"failed: {exc}"}
+        try:
+            t_cpu, nf, rows = oracle_time(w, CPU_BASELINE_FRAMES[c])
+            cpu = {"value": nf / t_cpu, "unit": UNIT, "cores": 1, "kind": "oracle",
+                   "sample": f"first {nf} of {B} frames of {w.name} ({rows} candidates), one pass, single thread, {t_cpu:.2f} s",
+                   "candidates_per_s": rows / t_cpu, "host_cpus": os.cpu_count()}
+        except Exception as exc:  # the baseline is reported, never required for the GPU numbers
+            cpu = {"value": None, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": f"failed: {exc}"}
 
+        ms_step = total_ms / K
+        configs[str(c)] = {"workload": CONFIG_DESC[c], "ms_per_step": ms_step, "frames_per_s": B / (ms_step * 1e-3),
+                           "candidates_per_s": total_cand / (ms_step * 1e-3),
+                           "a1_frac_of_hbm_peak": stages["a1_threshold_compact"]["frac_of_hbm_peak"],
+                           "a6_frac_of_hbm_peak": stages["a5a6_density"]["frac_of_hbm_peak"],
+                           "stages_ms": {nm: float(stage_ms[i]) for i, nm in enumerate(names)}, "steps": K,
+                           "kept": kept_n, "entering_nms": int(n_sorted.sum())}
+        e2e_ms = 1e3 * t_e2e / e2e_steps
         line = {
-            "metric": METRIC, "value": fps, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
-            "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32", "data": "synthetic",
+            "metric": METRIC, "value": fps, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "input_dtype": w.params["dtype"], "data": "synthetic",
             "config": {"workload": CONFIG_DESC[c], "frames_per_step_per_gpu": B, "candidates_per_step_per_gpu": total_cand,
                        "input_dtype": w.params["dtype"], "top_k": w.params["top_k"], "conf": w.params["conf_thresh"],
                        "iou": w.params["iou_thresh"], "sigma_cells": w.params["sigma_cells"],
-                       "l2": "flushed between steps (512 MB write outside the event pair)", "seed": "config_seed(c)+rank"},
+                       "l2": "cold and clean between steps (512 MB write, then 512 MB read, outside the event pair)",
+                       "seed": "config_seed(c)+rank"},
             "candidates_per_s": cps,
             "step_ms_min": float(step_ms.min()), "step_ms_median": float(np.median(step_ms)), "wall_s_timed_loop": t_wall,
             "e2e": {"value": frames_all * e2e_steps / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "ms_per_step": 1e3 * t_e2e / e2e_steps, "candidates_per_s": cand_all * e2e_steps / t_e2e,
+                    "ms_per_step": e2e_ms, "candidates_per_s": cand_all * e2e_steps / t_e2e,
+                    "pcie_floor_ms": max(h2d_ms, d2h_ms), "pcie_h2d_ms": h2d_ms, "pcie_d2h_ms": d2h_ms,
+                    "pcie_h2d_GB/s": h2d / (h2d_ms * 1e-3) / 1e9, "frac_of_pcie_floor": max(h2d_ms, d2h_ms) / e2e_ms,
                     "api": "ffpp_run_host (pinned host buffers, copies + sync inside the timed region)"},
-            "gpu_launches": 6 * K,
-            "warm_l2": {"ms_per_step": float(warm_ms.sum()), "frames_per_s": B / (float(warm_ms.sum()) * 1e-3),
-                        "stages_ms": {nm: float(warm_ms[i]) for i, nm in enumerate(names)},
-                        "a1_GB/s": alg_bytes["a1_threshold_compact"] / (float(warm_ms[1]) * 1e-3) / 1e9,
-                        "note": "no L2 flush between steps: inputs of <= 126 MB are served from L2, so a1's GB/s is not an HBM "
-                                "figure; per-GPU, this rank"},
+            "gpu_launches": ffpp.LAUNCHES_PER_RUN * K,
+            "launches_per_step": {"kernels": ffpp.LAUNCHES_PER_RUN, "memsets": 1, "descriptor_uploads": 0},
             "roofline": roofline,
             "step_roofline": step_roofline,
             "stages": stages,
+            "warm_l2": {"ms_per_step": float(warm_ms.sum()), "frames_per_s": B / (float(warm_ms.sum()) * 1e-3),
+                        "note": "no L2 flush between steps: inputs of <= 126 MB are served from L2, so a1's GB/s is not an HBM figure"},
+            "cold_dirty_l2": {"ms_per_step": float(dirty_ms.sum()),
+                              "note": "512 MB write only (round 1's regime): the first kernels compete with the write-back of dirty lines"},
+            "configs": configs,
             "cpu_baseline": cpu,
             "clocks": clocks,
             "workload_stats": {"survivors": int(n_surv.sum()), "entering_nms": int(n_sorted.sum()), "kept": kept_n,
@@ -430,7 +561,10 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-other-configs", action="store_true", help="skip the short measurements of the other four configs")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return respawn_under_torchrun(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

@@ -106,7 +106,8 @@ def _spec(W, H, lam, median, layout=0, ncomp=3, comp_sigma=60.0, frac=0.2, bg=(1
 
 
 def generate(name: str, specs: list[dict], *, dtype: str, conf: float, iou: float, top_k: int, sigma_cells: float,
-             seed: int, cell_px: int = 8, truncate_sigmas: float = 3.0, threads: int = 0) -> Workload:
+             seed: int, cell_px: int = 8, truncate_sigmas: float = 3.0, threads: int = 0,
+             iou_margin: float = 1e-5) -> Workload:
     """Generate one batch from explicit per-frame specs (see ``_spec``)."""
     lib = _load()
     B = len(specs)
@@ -116,7 +117,7 @@ def generate(name: str, specs: list[dict], *, dtype: str, conf: float, iou: floa
     for i, s in enumerate(STRIDES):
         pa.strides[i] = s
     pa.conf_thresh, pa.iou_thresh, pa.top_k = conf, iou, top_k
-    pa.jitter_px, pa.iou_margin, pa.threads = 1.5, 1e-5, threads
+    pa.jitter_px, pa.iou_margin, pa.threads = 1.5, iou_margin, threads
     arr = (_FrameSpec * max(B, 1))()
     for i, s in enumerate(specs):
         for k, v in s.items():
@@ -170,6 +171,8 @@ def config_specs(c: int, B: int | None = None):
     return specs, kw
 
 
-def make_config(c: int, seed_offset: int = 0, B: int | None = None, threads: int = 0) -> Workload:
+def make_config(c: int, seed_offset: int = 0, B: int | None = None, threads: int = 0, iou_margin: float = 1e-5) -> Workload:
+    """``iou_margin`` = 0 switches the IoU-margin rejection of SURVEY §8(d) step (7) off (parity cases only)."""
     specs, kw = config_specs(c, B)
-    return generate(f"config{c}" + (f"_B{B}" if B else ""), specs, seed=config_seed(c) + seed_offset, threads=threads, **kw)
+    return generate(f"config{c}" + (f"_B{B}" if B else ""), specs, seed=config_seed(c) + seed_offset, threads=threads,
+                    iou_margin=iou_margin, **kw)

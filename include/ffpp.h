@@ -41,7 +41,8 @@ typedef struct ffpp_params {
   int32_t dtype;           /* 0 = fp32, 1 = fp16 (IEEE binary16) rows of the raw head output                       */
   float conf_thresh;       /* threshold on sigmoid(logit), strict >, applied as logit > ln(c/(1-c))  (A7)          */
   float iou_thresh;        /* strict >; must be >= 0                                                   (A11)        */
-  int32_t top_k;           /* >= 1; at most 24576 (fp16 rows with N_f <= 65536) or 12288 (otherwise)               */
+  int32_t top_k;           /* >= 1; at most 24576 (fp16 rows with N_f <= 65536) or 12288 (otherwise): the top-K set of
+                              a frame (keys, spatial bins) is held in one SM's 227 KB of shared memory by a2/a4      */
   int32_t num_levels;      /* 1..4                                                                                  */
   int32_t strides[4];      /* ascending powers of two, e.g. {8,16,32}                                  (A5)         */
   int32_t cell_px;         /* density cell edge in pixels, e.g. 8                                                   */
@@ -55,8 +56,9 @@ typedef struct ffpp_params {
   int64_t nms_workspace_bytes; /* capacity of the NMS suppression-edge pool in bytes (4 per edge, shared out to the
                                   frames in proportion to min(N_f, top_k)); 0 = nms_edges_per_box edges per box       */
   int32_t nms_edges_per_box; /* 0 = 16.  An edge is one unordered pair {a, b} with IoU > iou_thresh; the flock
-                                workloads have 4-9 per box.  A frame that needs more than its share reports
-                                out_counts[f] = -1 and leaves its out_boxes / out_density rows undefined              */
+                                workloads have 4-9 per box.  The pool is a speed knob, never a correctness limit: a
+                                frame that needs more than its share is resolved by the pool-free overflow kernel
+                                (same result, bounded workspace, slower for that frame)                               */
   int32_t reserved_;
 } ffpp_params;
 
@@ -73,8 +75,11 @@ typedef struct ffpp_box {
 int ffpp_create(const ffpp_params* p /*HOST*/, ffpp_handle** out /*HOST*/);
 
 /* Run the whole path on one batch; everything is enqueued on `stream`, nothing is allocated, the host is never
- * synchronised (CUDA-graph capturable when the batch geometry equals the previous call's).  Results are complete
- * when `stream` reaches the point after the call; the caller synchronises.
+ * synchronised.  The frame descriptor table of a batch geometry (B, N_per_frame, frame_dims) is built on first
+ * sight, uploaded with one stream-ordered copy and cached in one of 32 device slots (least recently used slot is
+ * replaced), so alternating geometries cost nothing after their first call.  CUDA-graph capturable when the
+ * geometry is cached (run it once before capturing; an uncached geometry under capture returns FFPP_EINVAL).
+ * Results are complete when `stream` reaches the point after the call; the caller synchronises.
  *
  *   raw          DEVICE  [sum_f N_f][5] values (l, t, r, b in stride units, score logit) in params.dtype, frames
  *                        tightly concatenated in order (A22); 16-byte aligned base.  Read only.
@@ -96,9 +101,10 @@ int ffpp_run(ffpp_handle* h, const void* raw /*DEVICE*/, int32_t B, const int32_
 /* The same path with HOST buffers (the call a user without device buffers makes): copies raw host->device,
  * runs, copies the three outputs device->host through the handle's own staging, and synchronises `stream`
  * before returning.  raw / out_* are HOST pointers (pinned memory makes the copies asynchronous DMA; a pinned
- * out_boxes is written by one kernel through its device alias).  Batches of >= 32 MB and >= 16 frames are cut into
- * four runs of whole frames (frames are independent) so that the upload of the next run and the download of the
- * previous one, on two internal copy streams, overlap the kernels of the current run on `stream`. */
+ * out_boxes is written by one kernel through its device alias).  Batches of >= 16 MB and >= 16 frames are cut by
+ * bytes into up to 8 runs of whole frames (frames are independent) so that the upload of the next run and the
+ * download of the previous one, on two internal copy streams, overlap the kernels of the current run on
+ * `stream` (the D2H copy + CPU post-processing the paper blames; L308-310: streams as the remedy). */
 int ffpp_run_host(ffpp_handle* h, const void* raw /*HOST*/, int32_t B, const int32_t* N_per_frame /*HOST*/,
                   const int32_t* frame_dims /*HOST*/, void* stream, ffpp_box* out_boxes /*HOST*/,
                   int32_t* out_counts /*HOST*/, float* out_density /*HOST*/);
@@ -129,20 +135,6 @@ int ffpp_get_info(const ffpp_handle* h, ffpp_info* out /*HOST*/);
 #define FFPP_NUM_STAGES 6
 int ffpp_set_stage_timing(ffpp_handle* h, int32_t enable);
 int ffpp_get_stage_ms(ffpp_handle* h, float* ms_out /*HOST [FFPP_NUM_STAGES]*/);
-
-/* Test-only readback of per-stage intermediates of the LAST run (synchronises the device).
- *   what = 0: survivor count per frame after thresholding       dst HOST int32 [B]
- *   what = 1: sorted count per frame  min(n, top_k)             dst HOST int32 [B]
- *   what = 2: candidate indices of the top-K set in the order   dst HOST int32 [B][top_k] (rows past the count: -1)
- *             of O4 (the device holds the set with its keys in spatial order; the readback sorts by key on the host)
- *   what = 3: decoded boxes of the top-K set, same order        dst HOST float [B][top_k][4]
- * Not part of the contract of the path; used to localise a parity failure. */
-int ffpp_debug_read(ffpp_handle* h, int32_t what, void* dst /*HOST*/, int64_t dst_bytes);
-
-/* Calibration only: enqueue a plain coalesced read of `bytes` bytes of the DEVICE buffer `dev` (16-byte aligned) on
- * `stream`.  Computes nothing of the path; bench.py times it over the raw head output, under the same cold-cache
- * regime as stage a1, to report what a pure read of that size achieves on this GPU. */
-int ffpp_debug_stream_read(ffpp_handle* h, const void* dev /*DEVICE*/, int64_t bytes, void* stream);
 
 #ifdef __cplusplus
 }

@@ -1,7 +1,8 @@
 """paper_2512_07009_b200 — Python binding of libffpp (include/ffpp.h).
 
-Argument marshalling only: every step of the path (threshold/compaction, sort/top-K/decode, NMS bitmask,
-greedy sweep, density) runs in the hand-written sm_100a kernels of ``csrc/``.  PyTorch supplies device
+Argument marshalling only: every step of the path (threshold/compaction, top-K select + decode + spatial
+binning, NMS suppression pairs, greedy resolve + output gather, density) runs in the hand-written sm_100a
+kernels of ``csrc/``.  PyTorch supplies device
 memory and streams, nothing else.  There is no CPU fallback: if the CUDA library is missing or no
 sm_100 device is present, construction raises.
 
@@ -29,11 +30,14 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", 
 
 FFPP_OK, FFPP_EINVAL, FFPP_ECAPACITY, FFPP_ECUDA, FFPP_ENOMEM = 0, -1, -2, -3, -4
 NUM_STAGES = 6
-STAGE_NAMES = ["a0_schedule", "a1_threshold_compact", "a2_sort_topk_decode", "a3_nms_mask", "a4_nms_sweep", "a5a6_density"]
+STAGE_NAMES = ["a0_schedule", "a1_threshold_compact", "a2_select_decode_bin", "a3_nms_pairs", "a4_nms_resolve_emit", "a5a6_density"]
 
 STAGE_KERNELS = {"a0_schedule": "host scheduler + memset", "a1_threshold_compact": "k1_threshold_compact",
-                 "a2_sort_topk_decode": "k2_select_bin", "a3_nms_mask": "k3_nms_edges", "a4_nms_sweep": "k4_resolve_order + k4e_emit",
-                 "a5a6_density": "k5_density"}
+                 "a2_select_decode_bin": "k2_select_bin", "a3_nms_pairs": "k3_nms_edges (+ k3o_overflow)",
+                 "a4_nms_resolve_emit": "k4_resolve_order + k4e_emit", "a5a6_density": "k5_density"}
+# kernel launches of one ffpp_run (k1, k2, k3, k3o, k4, k4e, k5); plus one counter memset and, on first sight of a
+# batch geometry, one descriptor upload
+LAUNCHES_PER_RUN = 7
 
 # fp32 instructions per IoU pair of the all-pairs bitmask method (4 min/max, 2 sub, 2 clamp, 1 mul, area
 # add/sub, divide-or-multiply + compare = 12-16; 15 taken).  bench.py divides the fp32 lane rate by this to get the
@@ -43,7 +47,8 @@ NMS_ALU_OPS_PER_PAIR = 15
 BOX_DTYPE = np.dtype([("x1", "<f4"), ("y1", "<f4"), ("x2", "<f4"), ("y2", "<f4"), ("score", "<f4"), ("cand_index", "<i4")])
 
 EXPORTS = ["ffpp_create", "ffpp_run", "ffpp_run_host", "ffpp_destroy", "ffpp_last_error", "ffpp_get_info",
-           "ffpp_set_stage_timing", "ffpp_get_stage_ms", "ffpp_debug_read", "ffpp_debug_stream_read"]
+           "ffpp_set_stage_timing", "ffpp_get_stage_ms"]
+DEBUG_EXPORTS = ["ffpp_debug_read", "ffpp_debug_count_work", "ffpp_debug_stream_read"]     # include/ffpp_debug.h
 
 
 class FFPPParams(ctypes.Structure):
@@ -73,7 +78,7 @@ class FFPPError(RuntimeError):
 
 def build(force: bool = False, verbose: bool = False) -> str:
     """Compile csrc/ffpp.cu for sm_100a into libffpp.so next to this file (nvcc cross-compiles without a GPU)."""
-    srcs = [os.path.join(_CSRC, s) for s in _SOURCES] + [os.path.join(_INCLUDE, "ffpp.h")]
+    srcs = [os.path.join(_CSRC, s) for s in _SOURCES] + [os.path.join(_INCLUDE, "ffpp.h"), os.path.join(_INCLUDE, "ffpp_debug.h")]
     stale = not os.path.exists(_LIB) or any(os.path.getmtime(s) > os.path.getmtime(_LIB) for s in srcs)
     if force or stale:
         cmd = ["nvcc"] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", _LIB, os.path.join(_CSRC, "ffpp.cu")]
@@ -109,6 +114,8 @@ def load_library() -> ctypes.CDLL:
         L.ffpp_get_stage_ms.argtypes = [vp, vp]
         L.ffpp_debug_read.restype = ctypes.c_int
         L.ffpp_debug_read.argtypes = [vp, i32, vp, i64]
+        L.ffpp_debug_count_work.restype = ctypes.c_int
+        L.ffpp_debug_count_work.argtypes = [vp, i32]
         L.ffpp_debug_stream_read.restype = ctypes.c_int
         L.ffpp_debug_stream_read.argtypes = [vp, vp, i64, vp]
         _lib = L
@@ -283,10 +290,16 @@ class FFPP:
         self._check(self._lib.ffpp_debug_stream_read(self._h, dev_tensor.data_ptr(), dev_tensor.numel() * dev_tensor.element_size(),
                                                      st.cuda_stream))
 
+    def count_work(self, enable: bool):
+        """ffpp_debug_count_work: the next runs launch the counting instantiation of the a3 kernel."""
+        self._check(self._lib.ffpp_debug_count_work(self._h, 1 if enable else 0))
+
     def debug_read(self, what: int, B: int) -> np.ndarray:
         K = self.top_k
-        if what in (0, 1):
+        if what in (0, 1, 5):
             a = np.zeros(B, dtype=np.int32)
+        elif what == 4:
+            a = np.zeros(4, dtype=np.int64)
         elif what == 2:
             a = np.zeros((B, K), dtype=np.int32)
         else:

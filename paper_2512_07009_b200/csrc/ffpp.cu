@@ -8,6 +8,7 @@
 #include <string>
 #include <vector>
 
+#include "../../include/ffpp_debug.h"
 #include "ffpp_kernels.cuh"
 
 using namespace ffpp;
@@ -52,11 +53,10 @@ struct ffpp_handle {
   std::string err;
 
   // device workspace
-  uint8_t* d_meta = nullptr;
   void* d_surv_keys = nullptr;
   int* d_counters = nullptr;          // 4 x max_frames: survivor counts | top-K counts | edge counters | frame_err
   float4* d_sel_box = nullptr;        // a2 scratch: decoded boxes in selection order; 
-  float4* d_sp_box = nullptr;         // spatial (Hilbert) order, stride kpad per frame
+  float4* d_sp_box = nullptr;         // boxes in spatial order (row-major 16-px cell of the centre), stride kpad per frame
   float4* d_sp_sbox = nullptr;        // culling boxes
   void* d_sp_key = nullptr;
   uint8_t* d_hasin = nullptr;         // a3 -> a4: one byte per box, 1 = victim of at least one edge
@@ -67,22 +67,33 @@ struct ffpp_handle {
   uint32_t* d_edges = nullptr;
   uint32_t* d_hist32 = nullptr;       // a5: uint16 count per density cell, two per word
   int64_t workspace_bytes = 0;
-  // pinned staging for the descriptor table
-  uint8_t* h_meta = nullptr;
+  // a0: cached batch geometries.  A slot owns one device copy of the descriptor block; the host copy is built in a
+  // plain (pageable) vector and uploaded with cudaMemcpyAsync, which stages pageable memory before it returns: no
+  // pinned block to protect, hence no event and no host synchronisation.
   DeviceMeta ml;
-  cudaEvent_t meta_done = nullptr;    // last descriptor upload has been consumed by the copy engine
-  // geometry of the last batch (skip rebuild + upload when unchanged)
-  int last_B = -1;
-  std::vector<int32_t> last_N, last_dims;
-  int max_tiles = 0, max_nmax = 0;
-  int64_t total_cand = 0, total_cells = 0;
+  struct GeoSlot {
+    uint8_t* d_meta = nullptr;
+    uint64_t hash = 0, last_use = 0;
+    int B = -1;
+    std::vector<int32_t> N, dims;
+    int max_tiles = 0, max_nmax = 0;
+    int64_t total_cand = 0, total_cells = 0;
+  };
+  static constexpr int kGeoSlots = 32;
+  GeoSlot geo[kGeoSlots];
+  int cur = -1;                         // slot of the last run
+  uint64_t use_clock = 0;
+  std::vector<uint8_t> h_meta;          // host build area of the descriptor block
+  unsigned long long* d_work = nullptr; // a3 work counters (debug): culling tests, exact IoUs, edges
+  bool count_work = false;
   // host-buffer path staging (allocated on first ffpp_run_host)
   void* d_in = nullptr;
   ffpp_box* d_out_boxes = nullptr;
   int* d_out_counts = nullptr;
   float* d_out_density = nullptr;
   cudaStream_t s_h2d = nullptr, s_d2h = nullptr;     // copy streams of the chunked host path (created on first use)
-  cudaEvent_t ev_up[4] = {}, ev_run[4] = {};
+  static constexpr int kHostChunks = 8;
+  cudaEvent_t ev_up[kHostChunks] = {}, ev_run[kHostChunks] = {};
   // stage timing
   bool timing = false;
   cudaEvent_t ev[FFPP_NUM_STAGES + 1] = {};
@@ -120,17 +131,37 @@ int64_t frame_candidates(const ffpp_params& p, int W, int H) {
   return n;
 }
 
-// a0: validate the batch, (re)build the descriptor table, upload if the geometry changed.
+uint64_t geo_hash(int B, const int32_t* N, const int32_t* dims) {
+  uint64_t x = 0x9E3779B97F4A7C15ull ^ (uint64_t)B;
+  auto mix = [&](uint64_t v) { x ^= v + 0x9E3779B97F4A7C15ull + (x << 6) + (x >> 2); x *= 0xD6E8FEB86659FD93ull; x ^= x >> 32; };
+  for (int f = 0; f < B; ++f) { mix((uint32_t)N[f]); mix(((uint64_t)(uint32_t)dims[2 * f] << 32) | (uint32_t)dims[2 * f + 1]); }
+  return x;
+}
+
+// a0: find the batch geometry among the cached slots, else validate it, build its descriptor block and upload it
+// (one stream-ordered copy from pageable memory: no host synchronisation).  Sets h->cur.
 int schedule(ffpp_handle* h, int B, const int32_t* N, const int32_t* dims, cudaStream_t stream) {
   const ffpp_params& p = h->p;
-  if (B == h->last_B && std::memcmp(N, h->last_N.data(), sizeof(int32_t) * B) == 0 &&
-      std::memcmp(dims, h->last_dims.data(), sizeof(int32_t) * 2 * B) == 0)
-    return FFPP_OK;
-  // the previous upload may still be reading the pinned block
-  FFPP_CUDA(h, cudaEventSynchronize(h->meta_done));
-  h->last_B = -1;
-  FrameDesc* fr = reinterpret_cast<FrameDesc*>(h->h_meta + h->ml.frames_off);
-  int64_t* coff = reinterpret_cast<int64_t*>(h->h_meta + h->ml.cand_off_off);
+  const uint64_t hash = geo_hash(B, N, dims);
+  int lru = 0;
+  for (int s = 0; s < ffpp_handle::kGeoSlots; ++s) {
+    ffpp_handle::GeoSlot& g = h->geo[s];
+    if (g.B == B && g.hash == hash && std::memcmp(N, g.N.data(), sizeof(int32_t) * B) == 0 &&
+        std::memcmp(dims, g.dims.data(), sizeof(int32_t) * 2 * B) == 0) {
+      g.last_use = ++h->use_clock;
+      h->cur = s;
+      return FFPP_OK;
+    }
+    if (g.last_use < h->geo[lru].last_use) lru = s;
+  }
+  {
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(stream, &cap) == cudaSuccess && cap != cudaStreamCaptureStatusNone)
+      return fail(h, FFPP_EINVAL, "batch geometry not cached: run it once outside stream capture first");
+    cudaGetLastError();
+  }
+  FrameDesc* fr = reinterpret_cast<FrameDesc*>(h->h_meta.data() + h->ml.frames_off);
+  int64_t* coff = reinterpret_cast<int64_t*>(h->h_meta.data() + h->ml.cand_off_off);
   const int smax = p.strides[p.num_levels - 1];
   const int R = h->cst.radius;
   int64_t cand = 0, cells = 0, edges = 0;
@@ -170,38 +201,48 @@ int schedule(ffpp_handle* h, int B, const int32_t* N, const int32_t* dims, cudaS
     fr[f] = d;
     coff[f] = cand;
     cand += n; cells += (int64_t)d.gw * d.gh;
-    const int tiles = k5_tiles(d.gw, d.gh);
-    max_tiles = std::max(max_tiles, tiles);
+    d.k5_th = k5_tile_h(d.gw, d.gh);
+    d.k5_tiles = k5_tiles(d.gw, d.gh);
+    fr[f] = d;
+    max_tiles = std::max(max_tiles, (int)d.k5_tiles);
     max_nmax = std::max(max_nmax, (int)d.nmax);
   }
   coff[B] = cand;
   if (cand > p.max_total_candidates) return fail(h, FFPP_ECAPACITY, "sum N_f exceeds max_total_candidates");
+  size_t used = h->ml.block_frame_off;
   {
     // a1: first frame of every K1_BLOCK-row block of the flat candidate stream
-    int32_t* bf = reinterpret_cast<int32_t*>(h->h_meta + h->ml.block_frame_off);
+    int32_t* bf = reinterpret_cast<int32_t*>(h->h_meta.data() + h->ml.block_frame_off);
     int f = 0;
-    for (int64_t b = 0; b * K1_BLOCK < cand; ++b) {
+    int64_t b = 0;
+    for (; b * K1_BLOCK < cand; ++b) {
       while (f + 1 < B && coff[f + 1] <= b * K1_BLOCK) ++f;
       bf[b] = f;
     }
+    used += sizeof(int32_t) * (size_t)b;
   }
   if (cells > h->max_total_cells) return fail(h, FFPP_ECAPACITY, "density cells exceed max_total_cells");
   if (edges > h->edge_cap_total) return fail(h, FFPP_ECAPACITY, "suppression-edge pool exceeds nms_workspace_bytes");
-  FFPP_CUDA(h, cudaMemcpyAsync(h->d_meta, h->h_meta, h->ml.bytes, cudaMemcpyHostToDevice, stream));
-  FFPP_CUDA(h, cudaEventRecord(h->meta_done, stream));
-  h->last_B = B;
-  h->last_N.assign(N, N + B);
-  h->last_dims.assign(dims, dims + 2 * B);
-  h->max_tiles = max_tiles; h->max_nmax = max_nmax;
-  h->total_cand = cand; h->total_cells = cells;
+  ffpp_handle::GeoSlot& g = h->geo[lru];
+  g.B = -1;                                       // not valid until the copy is queued
+  used = (used + 15) & ~(size_t)15;
+  FFPP_CUDA(h, cudaMemcpyAsync(g.d_meta, h->h_meta.data(), used, cudaMemcpyHostToDevice, stream));
+  g.B = B; g.hash = hash;
+  g.N.assign(N, N + B);
+  g.dims.assign(dims, dims + 2 * B);
+  g.max_tiles = max_tiles; g.max_nmax = max_nmax;
+  g.total_cand = cand; g.total_cells = cells;
+  g.last_use = ++h->use_clock;
+  h->cur = lru;
   return FFPP_OK;
 }
 
 template <bool kHalf, typename KeyT>
 int launch_all(ffpp_handle* h, const void* raw, int B, cudaStream_t st, ffpp_box* out_boxes, int32_t* out_counts,
                float* out_density) {
-  const FrameDesc* frames = reinterpret_cast<const FrameDesc*>(h->d_meta + h->ml.frames_off);
-  const int64_t* coff = reinterpret_cast<const int64_t*>(h->d_meta + h->ml.cand_off_off);
+  const ffpp_handle::GeoSlot& g = h->geo[h->cur];
+  const FrameDesc* frames = reinterpret_cast<const FrameDesc*>(g.d_meta + h->ml.frames_off);
+  const int64_t* coff = reinterpret_cast<const int64_t*>(g.d_meta + h->ml.cand_off_off);
   const Consts& c = h->cst;
   const bool tm = h->timing;
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[1], st));
@@ -209,11 +250,11 @@ int launch_all(ffpp_handle* h, const void* raw, int B, cudaStream_t st, ffpp_box
   // a1
   {
     const int64_t row = kHalf ? 10 : 20;
-    const int64_t nchunks = (h->total_cand * row + K1_CHUNK_BYTES - 1) / K1_CHUNK_BYTES;
+    const int64_t nchunks = (g.total_cand * row + K1_CHUNK_BYTES - 1) / K1_CHUNK_BYTES;
     int64_t grid = (int64_t)h->sm_count * K1_CTAS_PER_SM;
     if (grid > nchunks) grid = nchunks;
     k1_threshold_compact<kHalf, KeyT><<<(unsigned)grid, K1_THREADS, K1_STAGES * K1_CHUNK_BYTES, st>>>(
-        static_cast<const uint8_t*>(raw), h->total_cand, B, coff, reinterpret_cast<const int32_t*>(h->d_meta + h->ml.block_frame_off),
+        static_cast<const uint8_t*>(raw), g.total_cand, B, coff, reinterpret_cast<const int32_t*>(g.d_meta + h->ml.block_frame_off),
         c.logit_thr, static_cast<KeyT*>(h->d_surv_keys), h->surv_cnt());
   }
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[2], st));
@@ -223,22 +264,31 @@ int launch_all(ffpp_handle* h, const void* raw, int B, cudaStream_t st, ffpp_box
       h->d_sel_box, h->d_sp_box, h->d_sp_sbox, static_cast<KeyT*>(h->d_sp_key), h->d_cellstart, h->n_sorted(), h->d_hist32,
       reinterpret_cast<uint32_t*>(h->d_hasin), h->sm_count);
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[3], st));
-  // a3
+  // a3 (+ the pool-free overflow path: its CTAs exit at once unless k3 flagged their frame)
   {
-    const dim3 g3((unsigned)((h->max_nmax + K3_THREADS - 1) / K3_THREADS), (unsigned)B);
-    if (g3.x > 0)
-      k3_nms_edges<KeyT><<<g3, K3_THREADS, 0, st>>>(frames, h->n_sorted(), h->d_sp_box, h->d_sp_sbox,
-                                                    static_cast<const KeyT*>(h->d_sp_key), h->d_cellstart, c,
-                                                    h->edge_ctr(), h->d_edges, h->d_hasin, h->frame_err());
+    const dim3 g3((unsigned)((g.max_nmax + K3_THREADS - 1) / K3_THREADS), (unsigned)B);
+    if (g3.x > 0) {
+      if (h->count_work)
+        k3_nms_edges<KeyT, true><<<g3, K3_THREADS, 0, st>>>(frames, h->n_sorted(), h->d_sp_box, h->d_sp_sbox,
+                                                            static_cast<const KeyT*>(h->d_sp_key), h->d_cellstart, c,
+                                                            h->edge_ctr(), h->d_edges, h->d_hasin, h->frame_err(), h->d_work);
+      else
+        k3_nms_edges<KeyT, false><<<g3, K3_THREADS, 0, st>>>(frames, h->n_sorted(), h->d_sp_box, h->d_sp_sbox,
+                                                             static_cast<const KeyT*>(h->d_sp_key), h->d_cellstart, c,
+                                                             h->edge_ctr(), h->d_edges, h->d_hasin, h->frame_err(), h->d_work);
+      k3o_overflow<KeyT><<<B, K3O_THREADS, (size_t)c.kpad, st>>>(frames, h->n_sorted(), h->d_sp_box, h->d_sp_sbox,
+                                                                static_cast<const KeyT*>(h->d_sp_key), h->d_cellstart, c,
+                                                                h->edge_ctr(), h->d_hasin, h->frame_err());
+    }
   }
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[4], st));
   // a4 (+ a5 histogram)
   k4_resolve_order<KeyT><<<B, K4_THREADS, k4_smem_bytes((size_t)c.top_k, (size_t)c.kpad, sizeof(KeyT)), st>>>(
       frames, h->n_sorted(), h->d_sp_box, static_cast<const KeyT*>(h->d_sp_key), h->edge_ctr(), h->d_edges,
-      reinterpret_cast<const uint32_t*>(h->d_hasin), h->frame_err(), c, h->sm_count, h->d_k4_scratch,
+      reinterpret_cast<const uint32_t*>(h->d_hasin), c, h->sm_count, h->d_k4_scratch,
       static_cast<KeyT*>(h->d_kept_key), h->d_kept_pos, out_counts);
   {
-    const dim3 g4e((unsigned)((h->max_nmax + K4E_THREADS - 1) / K4E_THREADS), (unsigned)B);
+    const dim3 g4e((unsigned)((g.max_nmax + K4E_THREADS - 1) / K4E_THREADS), (unsigned)B);
     if (g4e.x > 0)
       k4e_emit<KeyT><<<g4e, K4E_THREADS, 0, st>>>(frames, h->d_sp_box, static_cast<const KeyT*>(h->d_kept_key), h->d_kept_pos,
                                                   out_counts, c, out_boxes, h->d_hist32);
@@ -246,8 +296,8 @@ int launch_all(ffpp_handle* h, const void* raw, int B, cudaStream_t st, ffpp_box
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[5], st));
   // a6
   {
-    const dim3 g5((unsigned)h->max_tiles, (unsigned)B);
-    const size_t s5 = k5_smem_bytes(h->p.max_frame_w / h->p.cell_px, c.radius_t);
+    const dim3 g5((unsigned)g.max_tiles, (unsigned)B);
+    const size_t s5 = k5_smem_bytes(h->p.max_frame_w / h->p.cell_px, h->p.max_frame_h / h->p.cell_px, c.radius_t);
     const uint16_t* h16 = reinterpret_cast<const uint16_t*>(h->d_hist32);
     switch (c.radius_t) {
 #define FFPP_K5_CASE(RT) case RT: k5_density<RT><<<g5, K5_THREADS, s5, st>>>(frames, c, h16, out_density); break;
@@ -272,6 +322,7 @@ int set_kernel_attrs(ffpp_handle* h) {
   FFPP_CUDA(h, cudaFuncSetAttribute(k2_select_bin<kHalf, KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s2));
   const size_t s4 = k4_smem_bytes((size_t)h->p.top_k, (size_t)h->kpad, sizeof(KeyT));
   FFPP_CUDA(h, cudaFuncSetAttribute(k4_resolve_order<KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s4));
+  FFPP_CUDA(h, cudaFuncSetAttribute(k3o_overflow<KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->kpad));
   return FFPP_OK;
 }
 
@@ -378,7 +429,10 @@ int ffpp_create(const ffpp_params* p, ffpp_handle** out) {
     return ee;
   };
   const size_t KP = (size_t)h->kpad, F = (size_t)p->max_frames;
-  if ((e = dalloc((void**)&h->d_meta, h->ml.bytes)) != cudaSuccess ||
+  e = cudaSuccess;
+  for (int sl = 0; sl < ffpp_handle::kGeoSlots && e == cudaSuccess; ++sl) e = dalloc((void**)&h->geo[sl].d_meta, h->ml.bytes);
+  if (e != cudaSuccess ||
+      (e = dalloc((void**)&h->d_work, 4 * sizeof(unsigned long long))) != cudaSuccess ||
       (e = dalloc(&h->d_surv_keys, (size_t)p->max_total_candidates * h->key_bytes)) != cudaSuccess ||
       (e = dalloc((void**)&h->d_counters, (3 + kCntStride) * F * sizeof(int))) != cudaSuccess ||
       (e = dalloc((void**)&h->d_sel_box, F * KP * sizeof(float4))) != cudaSuccess ||
@@ -395,8 +449,8 @@ int ffpp_create(const ffpp_params* p, ffpp_handle** out) {
     cudaGetLastError();
     return bail(e == cudaErrorMemoryAllocation ? FFPP_ENOMEM : FFPP_ECUDA, std::string("workspace cudaMalloc: ") + cudaGetErrorString(e));
   }
-  if ((e = cudaMallocHost((void**)&h->h_meta, h->ml.bytes)) != cudaSuccess) return bail(FFPP_ENOMEM, std::string("cudaMallocHost: ") + cudaGetErrorString(e));
-  if ((e = cudaEventCreateWithFlags(&h->meta_done, cudaEventDisableTiming)) != cudaSuccess) return bail(FFPP_ECUDA, std::string("cudaEventCreate: ") + cudaGetErrorString(e));
+  h->h_meta.assign(h->ml.bytes, 0);
+  if ((e = cudaMemset(h->d_work, 0, 4 * sizeof(unsigned long long))) != cudaSuccess) return bail(FFPP_ECUDA, std::string("cudaMemset: ") + cudaGetErrorString(e));
   for (int i = 0; i <= FFPP_NUM_STAGES; ++i)
     if ((e = cudaEventCreate(&h->ev[i])) != cudaSuccess) return bail(FFPP_ECUDA, std::string("cudaEventCreate: ") + cudaGetErrorString(e));
   int rc;
@@ -405,7 +459,7 @@ int ffpp_create(const ffpp_params* p, ffpp_handle** out) {
   else rc = set_kernel_attrs<false, uint64_t>(h);
   if (rc != FFPP_OK) { std::string m = h->err; return bail(rc, m); }
   {
-    const size_t s5 = k5_smem_bytes(p->max_frame_w / p->cell_px, c.radius_t);
+    const size_t s5 = k5_smem_bytes(p->max_frame_w / p->cell_px, p->max_frame_h / p->cell_px, c.radius_t);
     e = cudaSuccess;
     switch (c.radius_t) {
 #define FFPP_K5_CASE(RT) case RT: e = cudaFuncSetAttribute(k5_density<RT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s5); break;
@@ -428,11 +482,14 @@ int ffpp_run(ffpp_handle* h, const void* raw, int32_t B, const int32_t* N_per_fr
   if (B > h->p.max_frames) return fail(h, FFPP_ECAPACITY, "B exceeds max_frames");
   if (reinterpret_cast<uintptr_t>(raw) & 15) return fail(h, FFPP_EINVAL, "raw must be 16-byte aligned");
   if (reinterpret_cast<uintptr_t>(out_boxes) & 7) return fail(h, FFPP_EINVAL, "out_boxes must be 8-byte aligned");
+  if ((reinterpret_cast<uintptr_t>(out_density) | reinterpret_cast<uintptr_t>(out_counts)) & 3)
+    return fail(h, FFPP_EINVAL, "out_counts / out_density must be 4-byte aligned");
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   if (h->timing) FFPP_CUDA(h, cudaEventRecord(h->ev[0], st));
   int rc = schedule(h, B, N_per_frame, frame_dims, st);
   if (rc != FFPP_OK) return rc;
   FFPP_CUDA(h, cudaMemsetAsync(h->d_counters, 0, sizeof(int) * (3 + kCntStride) * (size_t)h->p.max_frames, st));
+  if (h->count_work) FFPP_CUDA(h, cudaMemsetAsync(h->d_work, 0, 4 * sizeof(unsigned long long), st));
   if (h->half && h->key_bytes == 4) return launch_all<true, uint32_t>(h, raw, B, st, out_boxes, out_counts, out_density);
   if (h->half) return launch_all<true, uint64_t>(h, raw, B, st, out_boxes, out_counts, out_density);
   return launch_all<false, uint64_t>(h, raw, B, st, out_boxes, out_counts, out_density);
@@ -447,20 +504,31 @@ int ffpp_run_host(ffpp_handle* h, const void* raw, int32_t B, const int32_t* N_p
   if (B > h->p.max_frames) return fail(h, FFPP_ECAPACITY, "B exceeds max_frames");
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const size_t esz = h->half ? 2 : 4;
-  if (!h->d_in) {  // first use of the host path: its device staging (not part of ffpp_run's no-allocation promise)
-    const size_t K = (size_t)h->p.top_k, F = (size_t)h->p.max_frames;
-    FFPP_CUDA(h, cudaMalloc(&h->d_in, (size_t)h->p.max_total_candidates * 5 * esz + 16));
-    FFPP_CUDA(h, cudaMalloc((void**)&h->d_out_boxes, F * K * sizeof(ffpp_box)));
-    FFPP_CUDA(h, cudaMalloc((void**)&h->d_out_counts, F * sizeof(int)));
-    FFPP_CUDA(h, cudaMalloc((void**)&h->d_out_density, (size_t)h->max_total_cells * sizeof(float)));
-  }
+  // sizes are checked BEFORE anything is queued: they become byte counts of the uploads below
   int64_t cand = 0, cells = 0;
   for (int f = 0; f < B; ++f) {
+    const int W = frame_dims[2 * f], H = frame_dims[2 * f + 1];
+    if (W <= 0 || H <= 0) return fail(h, FFPP_EINVAL, "frame_dims: W and H must be positive");
+    if (N_per_frame[f] <= 0 || (int64_t)N_per_frame[f] != frame_candidates(h->p, W, H))
+      return fail(h, FFPP_EINVAL, "N_per_frame[f] != sum_l W*H/s_l^2");
     cand += N_per_frame[f];
-    cells += (int64_t)(frame_dims[2 * f] / h->p.cell_px) * (frame_dims[2 * f + 1] / h->p.cell_px);
+    cells += (int64_t)(W / h->p.cell_px) * (H / h->p.cell_px);
   }
   if (cand > h->p.max_total_candidates) return fail(h, FFPP_ECAPACITY, "sum N_f exceeds max_total_candidates");
   if (cells > h->max_total_cells) return fail(h, FFPP_ECAPACITY, "density cells exceed max_total_cells");
+  if (!h->d_in) {  // first use of the host path: its device staging (not part of ffpp_run's no-allocation promise), all or nothing
+    const size_t K = (size_t)h->p.top_k, F = (size_t)h->p.max_frames;
+    cudaError_t e;
+    if ((e = cudaMalloc(&h->d_in, (size_t)h->p.max_total_candidates * 5 * esz + 16)) != cudaSuccess ||
+        (e = cudaMalloc((void**)&h->d_out_boxes, F * K * sizeof(ffpp_box))) != cudaSuccess ||
+        (e = cudaMalloc((void**)&h->d_out_counts, F * sizeof(int))) != cudaSuccess ||
+        (e = cudaMalloc((void**)&h->d_out_density, (size_t)h->max_total_cells * sizeof(float) + 16)) != cudaSuccess) {
+      cudaGetLastError();
+      cudaFree(h->d_in); cudaFree(h->d_out_boxes); cudaFree(h->d_out_counts); cudaFree(h->d_out_density);
+      h->d_in = nullptr; h->d_out_boxes = nullptr; h->d_out_counts = nullptr; h->d_out_density = nullptr;
+      return fail(h, e == cudaErrorMemoryAllocation ? FFPP_ENOMEM : FFPP_ECUDA, std::string("host-path staging cudaMalloc: ") + cudaGetErrorString(e));
+    }
+  }
   // kept boxes: only rows [0, count) of each frame are defined.  A pinned (device-mapped) out_boxes is written by one
   // kernel through its device alias; a pageable one gets one copy per frame after the counts have arrived.
   const size_t K = (size_t)h->p.top_k;
@@ -472,17 +540,25 @@ int ffpp_run_host(ffpp_handle* h, const void* raw, int32_t B, const int32_t* N_p
     else
       cudaGetLastError();
   }
-  // Frames are independent, so a large batch is cut into up to kHostChunks runs of whole frames: the upload of run
-  // i+1 (copy stream) and the download of run i-1 (second copy stream) overlap the kernels of run i on `stream`.
-  // A run starts where the raw byte offset is a multiple of 16 (ffpp_run's alignment rule).
-  constexpr int kHostChunks = 4;
+  // Frames are independent, so a large batch is cut BY BYTES into up to kHostChunks runs of whole frames: the upload of
+  // run i+1 (copy stream) and the download of run i-1 (second copy stream) overlap the kernels of run i on `stream`.
+  // A run starts where the raw byte offset is a multiple of 16 (ffpp_run's alignment rule).  The last runs are the
+  // small ones: what is left after the final upload (its kernels + its download) is the un-overlapped tail.
+  constexpr int kHostChunks = ffpp_handle::kHostChunks;
+  static const int kShare[kHostChunks] = {3, 3, 3, 3, 3, 2, 2, 1};            // of 20: relative raw bytes of the runs
   const size_t row = 5 * esz;
   std::vector<int> cut{0};                                          // first frame of every run, then B
-  if (B >= 4 * kHostChunks && (size_t)cand * row >= ((size_t)32 << 20)) {
-    int64_t acc = 0;
-    int next = 1;
-    for (int f = 0; f < B && next < kHostChunks; ++f) {
-      if (f > cut.back() && acc * (int64_t)row % 16 == 0 && acc >= cand * next / kHostChunks) { cut.push_back(f); ++next; }
+  if (B >= 2 * kHostChunks && (size_t)cand * row >= ((size_t)16 << 20)) {
+    int64_t acc = 0, want = 0;
+    int next = 0;
+    want = cand * kShare[0] / 20;
+    for (int f = 0; f < B && next + 1 < kHostChunks; ++f) {
+      if (f > cut.back() && acc * (int64_t)row % 16 == 0 && acc >= want) {
+        cut.push_back(f); ++next;
+        int sh = 0;
+        for (int q = 0; q <= next; ++q) sh += kShare[q];
+        want = cand * sh / 20;
+      }
       acc += N_per_frame[f];
     }
   }
@@ -552,15 +628,14 @@ int ffpp_run_host(ffpp_handle* h, const void* raw, int32_t B, const int32_t* N_p
 
 int ffpp_destroy(ffpp_handle* h) {
   if (!h) return FFPP_OK;
-  cudaFree(h->d_meta); cudaFree(h->d_surv_keys); cudaFree(h->d_counters); cudaFree(h->d_sel_box); cudaFree(h->d_sp_box);
+  for (int sl = 0; sl < ffpp_handle::kGeoSlots; ++sl) cudaFree(h->geo[sl].d_meta);
+  cudaFree(h->d_work); cudaFree(h->d_surv_keys); cudaFree(h->d_counters); cudaFree(h->d_sel_box); cudaFree(h->d_sp_box);
   cudaFree(h->d_sp_sbox); cudaFree(h->d_sp_key); cudaFree(h->d_cellstart); cudaFree(h->d_hasin); cudaFree(h->d_k4_scratch); cudaFree(h->d_kept_key); cudaFree(h->d_kept_pos); cudaFree(h->d_edges);
   cudaFree(h->d_hist32);
   cudaFree(h->d_in); cudaFree(h->d_out_boxes); cudaFree(h->d_out_counts); cudaFree(h->d_out_density);
   if (h->s_h2d) cudaStreamDestroy(h->s_h2d);
   if (h->s_d2h) cudaStreamDestroy(h->s_d2h);
-  for (int i = 0; i < 4; ++i) { if (h->ev_up[i]) cudaEventDestroy(h->ev_up[i]); if (h->ev_run[i]) cudaEventDestroy(h->ev_run[i]); }
-  if (h->h_meta) cudaFreeHost(h->h_meta);
-  if (h->meta_done) cudaEventDestroy(h->meta_done);
+  for (int i = 0; i < ffpp_handle::kHostChunks; ++i) { if (h->ev_up[i]) cudaEventDestroy(h->ev_up[i]); if (h->ev_run[i]) cudaEventDestroy(h->ev_run[i]); }
   for (int i = 0; i <= FFPP_NUM_STAGES; ++i)
     if (h->ev[i]) cudaEventDestroy(h->ev[i]);
   delete h;
@@ -597,8 +672,8 @@ int ffpp_get_stage_ms(ffpp_handle* h, float* ms_out) {
 
 int ffpp_debug_read(ffpp_handle* h, int32_t what, void* dst, int64_t dst_bytes) {
   if (!h || !dst) return FFPP_EINVAL;
-  if (h->last_B < 0) return fail(h, FFPP_EINVAL, "no run to read back");
-  const int B = h->last_B;
+  if (h->cur < 0 || h->geo[h->cur].B < 0) return fail(h, FFPP_EINVAL, "no run to read back");
+  const int B = h->geo[h->cur].B;
   const size_t K = (size_t)h->p.top_k;
   FFPP_CUDA(h, cudaDeviceSynchronize());
   if (what == 0 || what == 1) {
@@ -607,6 +682,21 @@ int ffpp_debug_read(ffpp_handle* h, int32_t what, void* dst, int64_t dst_bytes) 
       FFPP_CUDA(h, cudaMemcpy2D(dst, sizeof(int), h->surv_cnt(), sizeof(int) * kCntStride, sizeof(int), (size_t)B, cudaMemcpyDeviceToHost));
     else
       FFPP_CUDA(h, cudaMemcpy(dst, h->n_sorted(), sizeof(int) * B, cudaMemcpyDeviceToHost));
+    return FFPP_OK;
+  }
+  if (what == 4) {
+    if (dst_bytes < (int64_t)(4 * sizeof(int64_t))) return fail(h, FFPP_EINVAL, "dst too small");
+    int64_t* d = static_cast<int64_t*>(dst);
+    FFPP_CUDA(h, cudaMemcpy(d, h->d_work, 3 * sizeof(int64_t), cudaMemcpyDeviceToHost));
+    std::vector<int> fe((size_t)B);
+    FFPP_CUDA(h, cudaMemcpy(fe.data(), h->frame_err(), sizeof(int) * B, cudaMemcpyDeviceToHost));
+    d[3] = 0;
+    for (int f = 0; f < B; ++f) d[3] += fe[(size_t)f] != 0;
+    return FFPP_OK;
+  }
+  if (what == 5) {
+    if (dst_bytes < (int64_t)(sizeof(int) * B)) return fail(h, FFPP_EINVAL, "dst too small");
+    FFPP_CUDA(h, cudaMemcpy(dst, h->frame_err(), sizeof(int) * B, cudaMemcpyDeviceToHost));
     return FFPP_OK;
   }
   if (what != 2 && what != 3) return fail(h, FFPP_EINVAL, "unknown debug selector");
@@ -643,6 +733,12 @@ int ffpp_debug_read(ffpp_handle* h, int32_t what, void* dst, int64_t dst_bytes) 
   }
   return FFPP_OK;
 
+}
+
+int ffpp_debug_count_work(ffpp_handle* h, int32_t enable) {
+  if (!h) return FFPP_EINVAL;
+  h->count_work = enable != 0;
+  return FFPP_OK;
 }
 
 int ffpp_debug_stream_read(ffpp_handle* h, const void* dev, int64_t bytes, void* stream) {

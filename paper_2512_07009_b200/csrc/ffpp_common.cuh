@@ -31,6 +31,7 @@ struct FrameDesc {
   int32_t cgw, cgh;                 // spatial cell grid (cgw * cgh <= kMaxCells), covers [0,W) x [0,H)
   int32_t lvl_start[kMaxLevels];    // first candidate of level l within the frame
   int32_t lvl_gw[kMaxLevels];       // W / s_l
+  int32_t k5_th, k5_tiles;          // a6: output rows per tile (multiple of 16) and tiles of this frame
 };
 
 // Method constants shared by all kernels (passed by value).
@@ -154,6 +155,12 @@ __device__ __forceinline__ void emit_kept(const FrameDesc& fd, const Consts& cst
     const int64_t h = fd.dens_off + (int64_t)cyi * fd.gw + cxi;
     atomicAdd(&hist32[h >> 1], 1u << (16 * (int)(h & 1)));
   }
+}
+
+__device__ __forceinline__ unsigned long long warp_sum_u64(unsigned long long v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
 }
 
 // ---- PTX helpers: mbarrier + 1-D bulk async copy (TMA engine, UBLKCP in SASS) ----

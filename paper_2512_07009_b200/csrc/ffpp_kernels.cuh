@@ -523,6 +523,7 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
 //      comes first in the order of O4 (smaller key); edges are staged per warp and appended to the frame's edge pool
 //      with one atomicAdd per flush, and the victim's "has a suppressor" byte is set (a plain store).
 // =====================================================================================================
+constexpr uint32_t ST_U = 0, ST_K = 1, ST_R = 2;   // box state of the greedy fixed point (a3 overflow path, a4)
 constexpr int K3_WARPS = 8;
 constexpr int K3_THREADS = 32 * K3_WARPS;
 constexpr int K3_QCAP = 96;                     // candidate queue: <= 31 left over + <= 64 pushed per step
@@ -536,7 +537,7 @@ struct K3Warp {
   uint32_t sb[K3_SCAP];
 };
 
-template <typename KeyT>
+template <typename KeyT, bool kCount>
 __global__ void __launch_bounds__(K3_THREADS) k3_nms_edges(const FrameDesc* __restrict__ frames,
                                                            const int* __restrict__ n_sorted,
                                                            const float4* __restrict__ sp_box,
@@ -544,8 +545,10 @@ __global__ void __launch_bounds__(K3_THREADS) k3_nms_edges(const FrameDesc* __re
                                                            const KeyT* __restrict__ sp_key,
                                                            const uint16_t* __restrict__ cellstart, Consts cst,
                                                            int* __restrict__ edge_ctr, uint32_t* __restrict__ edges,
-                                                           uint8_t* __restrict__ hasin, int* __restrict__ frame_err) {
+                                                           uint8_t* __restrict__ hasin, int* __restrict__ frame_err,
+                                                           unsigned long long* __restrict__ work_ctr) {
   __shared__ K3Warp<KeyT> s_w[K3_WARPS];
+  unsigned long long n_pre = 0, n_exact = 0, n_edge = 0;      // kCount only: this lane's culling tests / IoUs / edges
 
   const int f = blockIdx.y;
   const int n = n_sorted[f];
@@ -553,6 +556,7 @@ __global__ void __launch_bounds__(K3_THREADS) k3_nms_edges(const FrameDesc* __re
   if (p0 >= n) return;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   if (p0 + warp * 32 >= n) return;
+  if (!kCount && *reinterpret_cast<volatile int*>(&frame_err[f])) return;   // the frame already goes to k3o_overflow
   const FrameDesc* fd = &frames[f];
   const int cgw = fd->cgw, cgh = fd->cgh, hs = fd->hshift;
   const int64_t obase = (int64_t)f * cst.kpad;
@@ -594,7 +598,7 @@ __global__ void __launch_bounds__(K3_THREADS) k3_nms_edges(const FrameDesc* __re
     if (base + scnt <= fd->edge_cap) {
       for (int k = lane; k < scnt; k += 32) edges[fd->edge_off + base + k] = W.sb[k];
     } else if (lane == 0) {
-      frame_err[f] = 1;                            // pool exhausted (only when nms_workspace_bytes was set too low)
+      frame_err[f] = 1;                            // the frame's pool share is exhausted: k3o_overflow resolves the frame
     }
     scnt = 0;
     __syncwarp();
@@ -606,8 +610,10 @@ __global__ void __launch_bounds__(K3_THREADS) k3_nms_edges(const FrameDesc* __re
     if (lane < nb) {
       const uint32_t q = W.q[qcnt - nb + lane];
       const uint32_t al = q >> 16, b = q & 0xFFFFu;
+      if (kCount) ++n_exact;
       if (iou_exceeds(W.rowbox[al], fbox[b], cst)) {
         hit = true;
+        if (kCount) ++n_edge;
         const uint32_t pa = (uint32_t)row0 + al;
         ed = fkey[b] < W.rowkey[al] ? ((pa << 16) | b) : ((b << 16) | pa);
         hasin[obase + (ed >> 16)] = 1;             // a4 starts every box that is nobody's victim as kept
@@ -637,6 +643,7 @@ __global__ void __launch_bounds__(K3_THREADS) k3_nms_edges(const FrameDesc* __re
       const float4 sb1 = fsbox[two ? j + 1 : j];
       h0 = boxes_overlap(sa, sb0);
       h1 = two && boxes_overlap(sa, sb1);
+      if (kCount) n_pre += two ? 2 : 1;
     }
     const uint32_t b0 = __ballot_sync(0xffffffffu, h0), b1 = __ballot_sync(0xffffffffu, h1);
     if (b0 | b1) {
@@ -651,6 +658,84 @@ __global__ void __launch_bounds__(K3_THREADS) k3_nms_edges(const FrameDesc* __re
   }
   if (qcnt > 0) exact_batch(qcnt);
   flush();
+  if (kCount) {
+    n_pre = warp_sum_u64(n_pre); n_exact = warp_sum_u64(n_exact); n_edge = warp_sum_u64(n_edge);
+    if (lane == 0) { atomicAdd(&work_ctr[0], n_pre); atomicAdd(&work_ctr[1], n_exact); atomicAdd(&work_ctr[2], n_edge); }
+  }
+}
+
+// =====================================================================================================
+// a3/a4 overflow path — a frame whose suppression pairs do not fit its share of the edge pool (k3 raised frame_err[f]).
+// Greedy NMS is the unique fixed point of  kept(a) <=> no kept b before a with IoU(a,b) > thr;  this kernel iterates to
+// it WITHOUT storing pairs: one CTA per flagged frame (all other CTAs exit at once), one state byte per box in shared
+// memory, and per round every undecided box re-examines its partner window (the same cell window and culling-box
+// pretest as k3, both directions this time):
+//     some kept partner before it has IoU > thr          -> removed
+//     no undecided-or-kept partner before it has IoU > thr -> kept
+//     otherwise                                             -> stays undecided.
+// K and R are final, so a decision taken from states another thread is updating in the same round is still right
+// (chaotic iteration); the first undecided box of the order always decides, so the loop ends after at most
+// (longest chain of overlapping boxes with decreasing score) rounds.  Workspace: kpad bytes of shared memory, whatever
+// the input.  The result goes to a4 through the frame's hasin bytes (0 = kept, 3 = removed) with an empty edge list.
+// =====================================================================================================
+constexpr int K3O_THREADS = 1024;
+template <typename KeyT>
+__global__ void __launch_bounds__(K3O_THREADS) k3o_overflow(const FrameDesc* __restrict__ frames, const int* __restrict__ n_sorted,
+                                                            const float4* __restrict__ sp_box, const float4* __restrict__ sp_sbox,
+                                                            const KeyT* __restrict__ sp_key, const uint16_t* __restrict__ cellstart,
+                                                            Consts cst, int* __restrict__ edge_ctr, uint8_t* __restrict__ hasin,
+                                                            const int* __restrict__ frame_err) {
+  extern __shared__ __align__(16) uint8_t s_state[];          // kpad bytes
+  const int f = blockIdx.x;
+  if (!frame_err[f]) return;
+  const int n = n_sorted[f];
+  const int tid = threadIdx.x;
+  const FrameDesc* fd = &frames[f];
+  const int cgw = fd->cgw, cgh = fd->cgh, hs = fd->hshift;
+  const int64_t obase = (int64_t)f * cst.kpad;
+  const float4* fbox = sp_box + obase;
+  const float4* fsbox = sp_sbox + obase;
+  const KeyT* fkey = sp_key + obase;
+  const uint16_t* cs = cellstart + (int64_t)f * kCellStride;
+  volatile uint8_t* st = s_state;
+  for (int i = tid; i < n; i += K3O_THREADS) st[i] = (uint8_t)ST_U;
+  __syncthreads();
+  const float cmx = (float)((cgw << hs) - 1), cmy = (float)((cgh << hs) - 1);
+  for (;;) {
+    bool undecided = false;
+    for (int p = tid; p < n; p += K3O_THREADS) {
+      if (st[p] != ST_U) continue;
+      const float4 a = fbox[p];
+      const float4 sa = fsbox[p];
+      const KeyT ka = fkey[p];
+      const float cxa = box_centre(a.x, a.z), cya = box_centre(a.y, a.w);
+      const float ex = fmaxf(cst.rho * (a.z - a.x), 0.0f) * 1.001f + 1e-5f * (fabsf(a.x) + fabsf(a.z));
+      const float ey = fmaxf(cst.rho * (a.w - a.y), 0.0f) * 1.001f + 1e-5f * (fabsf(a.y) + fabsf(a.w));
+      const int Xlo = cell_coord(cxa - ex, cmx, hs), Xhi = cell_coord(cxa + ex, cmx, hs);
+      const int Ylo = cell_coord(cya - ey, cmy, hs), Yhi = cell_coord(cya + ey, cmy, hs);
+      bool removed = false, blocked = false;
+      for (int Y = Ylo; Y <= Yhi && !removed; ++Y) {
+        const uint16_t* r = cs + Y * cgw;
+        const int e = r[Xhi + 1];
+        for (int j = r[Xlo]; j < e; ++j) {
+          const uint32_t sj = st[j];
+          if (sj == ST_R || j == p) continue;
+          if (!(fkey[j] < ka)) continue;                       // only a box BEFORE a in the order of O4 can suppress it
+          if (!boxes_overlap(sa, fsbox[j])) continue;
+          if (!iou_exceeds(a, fbox[j], cst)) continue;
+          if (sj == ST_K) { removed = true; break; }
+          blocked = true;
+        }
+      }
+      if (removed) st[p] = (uint8_t)ST_R;
+      else if (!blocked) st[p] = (uint8_t)ST_K;
+      else undecided = true;
+    }
+    if (!__syncthreads_or(undecided)) break;
+  }
+  uint8_t* hz = hasin + obase;
+  for (int i = tid; i < n; i += K3O_THREADS) hz[i] = st[i] == ST_K ? 0 : 3;    // k4: st = hasin ^ 1 -> K (1) / R (2)
+  if (tid == 0) edge_ctr[f] = 0;
 }
 
 // =====================================================================================================
@@ -681,7 +766,6 @@ constexpr int K4_SMEM_BUDGET = 108 * 1024;       // dynamic shared memory per CT
 constexpr int K4_MAXPERM = 1024;                 // batches up to this many frames get the weight-ordered CTA -> frame map
 constexpr int K4_UNROLL = 8;
 constexpr int K4_BITONIC_MAX = 1024;             // kept sets up to this size take the bitonic network, larger ones LSD radix
-constexpr uint32_t ST_U = 0, ST_K = 1, ST_R = 2;
 
 struct K4Misc {
   int wsum[K4_WARPS];
@@ -858,7 +942,7 @@ template <typename KeyT>
 __global__ void __launch_bounds__(K4_THREADS, 2) k4_resolve_order(
     const FrameDesc* __restrict__ frames, const int* __restrict__ n_sorted, const float4* __restrict__ sp_box,
     const KeyT* __restrict__ sp_key, const int* __restrict__ edge_ctr, uint32_t* edges,
-    const uint32_t* __restrict__ hasin, const int* __restrict__ frame_err, Consts cst, int sm_count, uint8_t* __restrict__ scratch,
+    const uint32_t* __restrict__ hasin, Consts cst, int sm_count, uint8_t* __restrict__ scratch,
     KeyT* __restrict__ kept_key, uint16_t* __restrict__ kept_pos, int* __restrict__ out_counts) {
   extern __shared__ __align__(16) uint8_t smem[];
   __shared__ FrameDesc fd;
@@ -910,7 +994,6 @@ __global__ void __launch_bounds__(K4_THREADS, 2) k4_resolve_order(
     __syncthreads();
   }
   const int f = s_frame;
-  if (frame_err[f]) { if (tid == 0) out_counts[f] = -1; return; }
   FFPP_PHASE(f, 0);
   if (tid == 0) fd = frames[f];
   const int n = n_sorted[f];
@@ -918,7 +1001,8 @@ __global__ void __launch_bounds__(K4_THREADS, 2) k4_resolve_order(
   {
     const uint32_t* hin = hasin + obase / 4;
     for (int i = tid; i < kpad / 4; i += K4_THREADS) {
-      st32[i] = hin[i] ^ 0x01010101u;                                  // victim of some edge -> U, else K
+      st32[i] = hin[i] ^ 0x01010101u;                                  // victim of some edge (1) -> U, nobody's victim (0) -> K;
+                                                                       // overflow path: 0 -> K, 3 -> R, with an empty edge list
       rem32[i] = 0u;
       blk32[i] = 0u;
     }
@@ -1077,7 +1161,7 @@ __global__ void __launch_bounds__(K4E_THREADS) k4e_emit(const FrameDesc* __restr
                                                         ffpp_box* __restrict__ out_boxes, uint32_t* __restrict__ hist32) {
   const int f = blockIdx.y;
   const int r = blockIdx.x * K4E_THREADS + threadIdx.x;
-  if (r >= out_counts[f]) return;                               // also frames flagged -1
+  if (r >= out_counts[f]) return;
   const int64_t o = (int64_t)f * cst.top_k + r;
   const KeyT key = kept_key[o];
   const float4 bx = sp_box[(int64_t)f * cst.kpad + kept_pos[o]];
@@ -1087,131 +1171,271 @@ __global__ void __launch_bounds__(K4E_THREADS) k4e_emit(const FrameDesc* __restr
 // =====================================================================================================
 // a6 — density convolution (north_star (d); the paper's grid-cell x bird loop,
 // PAPER.md:L203-208, restated as histogram + separable convolution).
-// One CTA per strip of K5_TH output rows x up to K5_TW columns of one frame.  The y pass runs FIRST, straight from
-// the uint16 histogram in global memory (L2-resident: a2/a4 wrote it microseconds earlier): a thread owns one
-// column and eight consecutive output rows, reads the 8 + 2R histogram rows it needs through the reflect fold
-// (fold(i,n) = -i-1 | 2n-1-i, the half-sample symmetric extension), and keeps the eight sums in registers; the
-// result goes to shared memory for the strip's columns plus R folded halo columns per side.  The x pass then reads
-// 8 + 2R consecutive floats of one row (float4 loads, row pitch = 4 mod 32 so a quarter warp of eight rows is
-// conflict-free), produces eight consecutive outputs and writes them as one 32-byte sector.  Because the y pass
-// comes first, nothing is computed for halo ROWS: the work is exactly 2(2R+1) FMAs per cell plus 2R/TW for the
-// halo columns.  The tap loops are fully unrolled for the compile-time radius RT >= R (taps zero-padded to RT), so
-// there is no window shifting and every tap is a constant-bank operand.
-// HBM traffic: 2 bytes per cell of histogram (mostly L2 hits) + one 4-byte store per cell.
+// One CTA per tile of th output rows x up to K5_TW output columns of one frame; th (a multiple of 16, chosen per grid
+// width by the host scheduler, FrameDesc::k5_th) makes a tile ~8 k cells whatever the grid width.  Everything after one
+// coalesced read of the uint16 histogram happens in shared memory:
+//  (1) stage: rows y0-RT .. y0+th+RT-1 of the histogram (reflect-folded at the top / bottom of the grid) are copied
+//      as they are, 16 bytes per cp.async (LDGSTS: asynchronous, no register staging);
+//  (2) y pass: a thread owns TWO adjacent columns and 16 consecutive output rows: one 32-bit shared load brings a
+//      pair of counts, two byte-permutes + two subtractions turn them into floats (the 2^23 trick: full-rate ALU, no
+//      I2F), and the 16 pairs of sums are updated with packed fma.rn.f32x2 (FFMA2: two fp32 FMAs per issue slot; the
+//      (w_k, w_k) tap pairs stay in registers).  Columns outside the grid are not computed: the reflect border makes
+//      them copies of columns inside, filled in by a mirror pass, so the y pass does exactly (2R+1) FMAs per cell;
+//  (3) x pass: a thread reads 8 + 2 RT consecutive floats of one row (16-byte loads, row pitch = 4 mod 32 so a quarter
+//      warp of eight rows is conflict-free) and produces eight consecutive outputs; the taps are consumed two at a
+//      time, (w_k, w_k+1) x (v_j, v_j+1) on the aligned register pairs the loads deliver (the even / odd partial sums
+//      are added at the end), again FFMA2; one 32-byte sector is written per thread (two 16-byte stores when the
+//      address allows, whatever the caller's base pointer).
+// Radii above K5_PACKED_MAX_RT (tap pairs would not fit the register file) take scalar FMAs with constant-bank taps.
+// The tap loops are fully unrolled for the compile-time radius bucket RT >= R (taps zero-padded to RT).
+// HBM traffic: 2 bytes per cell of histogram (L2 hits: a4 wrote it microseconds earlier) + one 4-byte store per cell.
 // =====================================================================================================
 constexpr int K5_THREADS = 256;
-constexpr int K5_TH = 16;                       // output rows per CTA (two 8-row register blocks)
-constexpr int K5_TW = 512;                      // output columns per CTA at most (wider grids are tiled in x)
+constexpr int K5_TW = 256;                      // output columns per CTA at most (wider grids are tiled in x)
+constexpr int K5_PACKED_MAX_RT = 10;
 
 __host__ __device__ inline int k5_tile_w(int gw) { return gw < K5_TW ? ((gw + 7) & ~7) : K5_TW; }      // multiple of 8
-__host__ __device__ inline int k5_pitch(int tw, int RT) {                 // >= tw + 2 RT + 2, = 4 mod 32
-  const int need = tw + 2 * RT + 2;
+__host__ __device__ inline int k5_tile_h(int gw, int gh) {                // multiple of 16: ~one y-pass unit per thread
+  const int npair = k5_tile_w(gw) / 2;
+  int nb = (K5_THREADS + npair / 2) / npair;
+  if (nb < 1) nb = 1;
+  const int cap = (gh + 15) & ~15;
+  return 16 * nb < cap ? 16 * nb : cap;
+}
+__host__ __device__ inline int k5_pitch_t(int tw, int RT) {               // >= tw + 2 RT + 4, = 4 mod 32
+  const int need = tw + 2 * RT + 4;
   return ((need - 4 + 31) / 32) * 32 + 4;
 }
-__host__ __device__ inline size_t k5_smem_bytes(int gw_max, int RT) {
-  return sizeof(float) * (size_t)K5_TH * k5_pitch(k5_tile_w(gw_max), RT);
+__host__ __device__ inline int k5_pitch_h(int tw, int RT) { return (tw + 2 * RT + 7 + 8 + 7) & ~7; }  // staged uint16 columns, multiple of 8
+__host__ __device__ inline size_t k5_tile_smem(int tw, int th, int RT) {
+  const size_t hb = (sizeof(uint16_t) * (size_t)(th + 2 * RT) * k5_pitch_h(tw, RT) + 15) & ~(size_t)15;
+  return hb + sizeof(float) * (size_t)th * k5_pitch_t(tw, RT);
 }
+__host__ __device__ inline size_t k5_smem_bytes(int gw_max, int gh_max, int RT) {   // largest tile any grid up to gw_max x gh_max needs
+  size_t m = 0;
+  for (int gw = 8; gw <= ((gw_max + 7) & ~7); gw += 8) {
+    const size_t b = k5_tile_smem(k5_tile_w(gw), k5_tile_h(gw, gh_max), RT);
+    if (b > m) m = b;
+  }
+  return m;
+}
+__host__ __device__ inline int k5_tiles_x(int gw) { const int tw = k5_tile_w(gw); return (gw + tw - 1) / tw; }
 __host__ __device__ inline int k5_tiles(int gw, int gh) {
-  const int tw = k5_tile_w(gw);
-  return ((gw + tw - 1) / tw) * ((gh + K5_TH - 1) / K5_TH);
+  const int th = k5_tile_h(gw, gh);
+  return k5_tiles_x(gw) * ((gh + th - 1) / th);
 }
 
 __device__ __forceinline__ int k5_fold(int i, const int n) {
   i = i < 0 ? -i - 1 : (i >= n ? 2 * n - 1 - i : i);
   return min(max(i, 0), n - 1);                  // beyond one fold only zero-padded taps look: any in-range cell will do
 }
+__device__ __forceinline__ void cp_async16(void* dst_smem, const void* src_gmem) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst_smem)), "l"(src_gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+// u / d for 0 <= u < 2^20 with inv = 1.0f / d: (u + 0.5) / d is at least 0.5 / d away from every integer, far more than
+// the rounding error of the product
+__device__ __forceinline__ int fast_div(const int u, const float inv) { return (int)(((float)u + 0.5f) * inv); }
+// packed fp32 pairs (FFMA2)
+__device__ __forceinline__ unsigned long long pk2(const float lo, const float hi) {
+  unsigned long long r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r;
+}
+__device__ __forceinline__ void unpk2(const unsigned long long v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ unsigned long long fma2(const unsigned long long a, const unsigned long long b, const unsigned long long c) {
+  unsigned long long d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d;
+}
 
 template <int RT>
 __global__ void __launch_bounds__(K5_THREADS) k5_density(const FrameDesc* __restrict__ frames, Consts cst,
                                                          const uint16_t* __restrict__ hist16,
                                                          float* __restrict__ out_density) {
-  extern __shared__ __align__(16) float s_t[];              // [K5_TH][P]: y-pass result, column c <-> gx = x0 - RT + c
+  extern __shared__ __align__(16) uint8_t s_k5[];
+  constexpr bool kPacked = RT <= K5_PACKED_MAX_RT;
   const int f = blockIdx.y;
   const FrameDesc* fd = &frames[f];
+  if ((int)blockIdx.x >= fd->k5_tiles) return;
   const int gw = fd->gw, gh = fd->gh;
-  const int tw = k5_tile_w(gw);
-  const int tiles_y = (gh + K5_TH - 1) / K5_TH;
+  const int tw = k5_tile_w(gw), th = fd->k5_th;
   int ty = (int)blockIdx.x, tx = 0;
-  if (gw > tw) {                                            // grids wider than one tile (> K5_TW columns) only
-    const int tiles_x = (gw + tw - 1) / tw;
-    ty = (int)blockIdx.x / tiles_x; tx = (int)blockIdx.x - ty * tiles_x;
-  }
-  if (ty >= tiles_y) return;
-  const int x0 = tx * tw, y0 = ty * K5_TH;
-  const int P = k5_pitch(tw, RT);
-  const int twh = tw + 2 * RT;
+  if (gw > tw) { const int tiles_x = (gw + tw - 1) / tw; ty = (int)blockIdx.x / tiles_x; tx = (int)blockIdx.x - ty * tiles_x; }
+  const int x0 = tx * tw, y0 = ty * th;
+  const int x1 = min(gw, x0 + tw);
+  const int cx0 = tx > 0 ? x0 - RT : 0, cx1 = min(gw, x1 + (x1 < gw ? RT : 0));   // columns the y pass must compute
+  const int sx0 = cx0 & ~7;                                  // first staged column (16-byte copies)
+  const int Ph = k5_pitch_h(tw, RT), Pt = k5_pitch_t(tw, RT);
+  uint16_t* s_h = reinterpret_cast<uint16_t*>(s_k5);         // [th + 2 RT][Ph]: staged histogram rows, column gx - sx0
+  float* s_t = reinterpret_cast<float*>(s_k5 + ((sizeof(uint16_t) * (size_t)(th + 2 * RT) * Ph + 15) & ~(size_t)15));
+  constexpr int OD = RT & 1;                                 // s_t[y][ct]: ct = gx - (x0 - RT) + OD, so even gx <-> even ct
   const int tid = threadIdx.x;
   const uint16_t* hsrc = hist16 + fd->dens_off;
-  constexpr int NW = 8 + 2 * RT;                            // window of one 8-output block
 
-  // ---- y pass: a thread owns column c and walks the strip's 8-row blocks ----
-  for (int c = tid; c < twh; c += K5_THREADS) {
-   const int gx = k5_fold(x0 - RT + c, gw);
-   for (int q = 0; q < K5_TH / 8; ++q) {
-    const int yb = y0 + 8 * q - RT;
-    float acc[8];
-#pragma unroll
-    for (int m = 0; m < 8; ++m) acc[m] = 0.0f;
-    const uint16_t* col = hsrc + gx;
-    if (yb >= 0 && yb + NW <= gh) {                         // interior block: rows yb .. yb + NW - 1, no fold
-      const uint16_t* pr = col + yb * gw;
-#pragma unroll
-      for (int r = 0; r < NW; ++r) {
-        const float v = (float)pr[r * gw];
-#pragma unroll
-        for (int m = 0; m < 8; ++m) {
-          const int k = r - m;                              // compile-time after unrolling
-          if (k >= 0 && k <= 2 * RT) acc[m] = fmaf(cst.taps_pad[k], v, acc[m]);
-        }
-      }
-    } else {
-#pragma unroll
-      for (int r = 0; r < NW; ++r) {
-        const float v = (float)col[k5_fold(yb + r, gh) * gw];
-#pragma unroll
-        for (int m = 0; m < 8; ++m) {
-          const int k = r - m;
-          if (k >= 0 && k <= 2 * RT) acc[m] = fmaf(cst.taps_pad[k], v, acc[m]);
-        }
-      }
-    }
-#pragma unroll
-    for (int m = 0; m < 8; ++m) s_t[(8 * q + m) * P + c] = acc[m];
-   }
-  }
-  if (tid < 2 * K5_TH) s_t[(tid >> 1) * P + twh + (tid & 1)] = 0.0f;     // the two slack columns the float4 loads touch
-  __syncthreads();
-
-  // ---- x pass: unit = (row y, 8-column group g); consecutive lanes take consecutive rows ----
-  float* out = out_density + fd->dens_off;
-  const bool vec_ok = ((fd->dens_off | (int64_t)gw) & 3) == 0;
-  for (int u = tid; u < K5_TH * (tw / 8); u += K5_THREADS) {
-    const int g = u / K5_TH, y = u - g * K5_TH;
-    const float4* row4 = reinterpret_cast<const float4*>(s_t + y * P + 8 * g);
-    float win[(NW + 3) & ~3];
-#pragma unroll
-    for (int i = 0; i < (NW + 3) / 4; ++i) {
-      const float4 t = row4[i];
-      win[4 * i] = t.x; win[4 * i + 1] = t.y; win[4 * i + 2] = t.z; win[4 * i + 3] = t.w;
-    }
-    float acc[8];
-#pragma unroll
-    for (int m = 0; m < 8; ++m) {
-      acc[m] = 0.0f;
-#pragma unroll
-      for (int k = 0; k <= 2 * RT; ++k) acc[m] = fmaf(cst.taps_pad[k], win[m + k], acc[m]);
-    }
-    const int gy = y0 + y, gx = x0 + 8 * g;
-    if (gy < gh) {
-      float* dst = out + (int64_t)gy * gw + gx;
-      if (vec_ok && gx + 8 <= gw) {
-        reinterpret_cast<float4*>(dst)[0] = make_float4(acc[0], acc[1], acc[2], acc[3]);
-        reinterpret_cast<float4*>(dst)[1] = make_float4(acc[4], acc[5], acc[6], acc[7]);
+  // ---- (1) stage: 8 cells (16 bytes) per copy ----
+  {
+    const int ng = (cx1 - sx0 + 7) >> 3;                    // 8-column groups per row
+    const int nrows = th + 2 * RT;
+    const float inv = 1.0f / (float)ng;
+    const bool vec = (((uintptr_t)hsrc & 15) == 0) && ((gw & 7) == 0);
+    for (int u = tid; u < ng * nrows; u += K5_THREADS) {
+      const int r = fast_div(u, inv), g = u - r * ng;
+      const int gy = k5_fold(y0 - RT + r, gh);
+      const int gx = sx0 + 8 * g;
+      const uint16_t* src = hsrc + gy * gw + gx;
+      uint16_t* dst = s_h + r * Ph + 8 * g;
+      if (vec) {                                            // gw % 8 == 0: a group never straddles the row end
+        cp_async16(dst, src);
       } else {
 #pragma unroll
-        for (int m = 0; m < 8; ++m)
-          if (gx + m < gw) dst[m] = acc[m];
+        for (int e = 0; e < 8; ++e) dst[e] = gx + e < gw ? src[e] : (uint16_t)0;
       }
+    }
+    cp_async_wait_all();
+  }
+  __syncthreads();
+
+  // ---- (2) y pass ----
+  {
+    const int px0 = cx0 & ~1;                               // pairs start on an even column (>= sx0)
+    const int npair = (cx1 - px0 + 1) >> 1;
+    const float inv = 1.0f / (float)npair;
+    if constexpr (kPacked) {
+      constexpr int RB = 16, NW = RB + 2 * RT;
+      unsigned long long wp[2 * RT + 1];
+#pragma unroll
+      for (int k = 0; k <= 2 * RT; ++k) wp[k] = pk2(cst.taps_pad[k], cst.taps_pad[k]);
+      for (int u = tid; u < npair * (th / RB); u += K5_THREADS) {
+        const int q = fast_div(u, inv), c = u - q * npair;
+        if (y0 + RB * q >= gh) continue;                    // a block of rows below the grid (last tile of a frame)
+        const uint32_t* col = reinterpret_cast<const uint32_t*>(s_h + (RB * q) * Ph + (px0 - sx0) + 2 * c);
+        unsigned long long acc[RB];
+#pragma unroll
+        for (int m = 0; m < RB; ++m) acc[m] = 0ull;
+#pragma unroll
+        for (int r = 0; r < NW; ++r) {
+          const uint32_t v = col[r * (Ph / 2)];
+          // count -> float without I2F: 0x4B000000 | c is the float 2^23 + c
+          const float v0 = __uint_as_float(__byte_perm(v, 0x4B000000u, 0x7610)) - 8388608.0f;
+          const float v1 = __uint_as_float(__byte_perm(v, 0x4B000000u, 0x7632)) - 8388608.0f;
+          const unsigned long long vv = pk2(v0, v1);
+#pragma unroll
+          for (int m = 0; m < RB; ++m) {
+            const int k = r - m;                            // compile-time after unrolling
+            if (k >= 0 && k <= 2 * RT) acc[m] = fma2(wp[k], vv, acc[m]);
+          }
+        }
+        unsigned long long* dst = reinterpret_cast<unsigned long long*>(s_t + (RB * q) * Pt + (px0 - (x0 - RT) + OD) + 2 * c);
+#pragma unroll
+        for (int m = 0; m < RB; ++m) dst[m * (Pt / 2)] = acc[m];
+      }
+    } else {
+      constexpr int RB = 8, NW = RB + 2 * RT;
+      for (int u = tid; u < npair * (th / RB); u += K5_THREADS) {
+        const int q = fast_div(u, inv), c = u - q * npair;
+        if (y0 + RB * q >= gh) continue;
+        const uint32_t* col = reinterpret_cast<const uint32_t*>(s_h + (RB * q) * Ph + (px0 - sx0) + 2 * c);
+        float a0[RB], a1[RB];
+#pragma unroll
+        for (int m = 0; m < RB; ++m) { a0[m] = 0.0f; a1[m] = 0.0f; }
+#pragma unroll
+        for (int r = 0; r < NW; ++r) {
+          const uint32_t v = col[r * (Ph / 2)];
+          const float v0 = __uint_as_float(__byte_perm(v, 0x4B000000u, 0x7610)) - 8388608.0f;
+          const float v1 = __uint_as_float(__byte_perm(v, 0x4B000000u, 0x7632)) - 8388608.0f;
+#pragma unroll
+          for (int m = 0; m < RB; ++m) {
+            const int k = r - m;
+            if (k >= 0 && k <= 2 * RT) { a0[m] = fmaf(cst.taps_pad[k], v0, a0[m]); a1[m] = fmaf(cst.taps_pad[k], v1, a1[m]); }
+          }
+        }
+        float2* dst = reinterpret_cast<float2*>(s_t + (RB * q) * Pt + (px0 - (x0 - RT) + OD) + 2 * c);
+#pragma unroll
+        for (int m = 0; m < RB; ++m) dst[m * (Pt / 2)] = make_float2(a0[m], a1[m]);
+      }
+    }
+  }
+  __syncthreads();
+  // mirror pass: the columns of the window that lie outside the grid are reflections of computed ones
+  {
+    const int nct = (x1 - x0) + 2 * RT;
+    const int lo = cx0 - (x0 - RT), hi = cx1 - (x0 - RT);   // computed range, in window columns
+    const int nfill = lo + (nct - hi);
+    if (nfill) {                                            // block-uniform
+      const float inv = 1.0f / (float)nfill;
+      for (int u = tid; u < nfill * th; u += K5_THREADS) {
+        const int y = fast_div(u, inv), e = u - y * nfill;
+        const int wc = e < lo ? e : hi + (e - lo);
+        const int gx = min(max(k5_fold(x0 - RT + wc, gw), cx0), cx1 - 1);
+        s_t[y * Pt + wc + OD] = s_t[y * Pt + (gx - (x0 - RT)) + OD];
+      }
+      __syncthreads();
+    }
+  }
+
+  // ---- (3) x pass: unit = (row y, 8-column group g); consecutive lanes take consecutive rows ----
+  float* out = out_density + fd->dens_off;
+  constexpr int NWX = 8 + 2 * RT;                           // window of one 8-output block
+  constexpr int NL = (NWX + OD + 3) / 4;
+  const float inv_th = 1.0f / (float)th;
+  unsigned long long wE[kPacked ? RT : 1], wO[kPacked ? RT : 1];
+  if constexpr (kPacked) {
+#pragma unroll
+    for (int j = 0; j < RT; ++j) {
+      wE[j] = pk2(cst.taps_pad[2 * j], cst.taps_pad[2 * j + 1]);
+      wO[j] = pk2(cst.taps_pad[2 * j + 1], cst.taps_pad[2 * j + 2]);
+    }
+  }
+  for (int u = tid; u < th * (tw / 8); u += K5_THREADS) {
+    const int g = fast_div(u, inv_th), y = u - g * th;
+    const int gy = y0 + y, gx = x0 + 8 * g;
+    if (gy >= gh || gx >= gw) continue;
+    float acc[8];
+    if constexpr (kPacked) {
+      const ulonglong2* row2 = reinterpret_cast<const ulonglong2*>(s_t + y * Pt + 8 * g);
+      unsigned long long P[2 * NL];                         // P[i] = (v[2i], v[2i+1])
+#pragma unroll
+      for (int i = 0; i < NL; ++i) { const ulonglong2 t = row2[i]; P[2 * i] = t.x; P[2 * i + 1] = t.y; }
+#pragma unroll
+      for (int m = 0; m < 8; ++m) {
+        constexpr int dummy = 0; (void)dummy;
+        const int s0 = OD + m;                              // window index of tap 0 (compile-time after unrolling)
+        unsigned long long a = 0ull;
+        float lo, hi, single;
+        if ((s0 & 1) == 0) {                                // taps (0,1), (2,3), ... on aligned pairs; tap 2 RT alone
+#pragma unroll
+          for (int j = 0; j < RT; ++j) a = fma2(wE[j], P[s0 / 2 + j], a);
+          unpk2(P[s0 / 2 + RT], lo, hi);
+          single = cst.taps_pad[2 * RT] * lo;
+        } else {                                            // tap 0 alone; taps (1,2), (3,4), ... on aligned pairs
+#pragma unroll
+          for (int j = 0; j < RT; ++j) a = fma2(wO[j], P[(s0 + 1) / 2 + j], a);
+          unpk2(P[(s0 - 1) / 2], lo, hi);
+          single = cst.taps_pad[0] * hi;
+        }
+        unpk2(a, lo, hi);
+        acc[m] = (lo + hi) + single;
+      }
+    } else {
+      const float4* row4 = reinterpret_cast<const float4*>(s_t + y * Pt + 8 * g);
+      float win[4 * NL];
+#pragma unroll
+      for (int i = 0; i < NL; ++i) {
+        const float4 t = row4[i];
+        win[4 * i] = t.x; win[4 * i + 1] = t.y; win[4 * i + 2] = t.z; win[4 * i + 3] = t.w;
+      }
+#pragma unroll
+      for (int m = 0; m < 8; ++m) {
+        acc[m] = 0.0f;
+#pragma unroll
+        for (int k = 0; k <= 2 * RT; ++k) acc[m] = fmaf(cst.taps_pad[k], win[OD + m + k], acc[m]);
+      }
+    }
+    float* dst = out + gy * gw + gx;
+    if ((((uintptr_t)dst & 15) == 0) && gx + 8 <= gw) {
+      reinterpret_cast<float4*>(dst)[0] = make_float4(acc[0], acc[1], acc[2], acc[3]);
+      reinterpret_cast<float4*>(dst)[1] = make_float4(acc[4], acc[5], acc[6], acc[7]);
+    } else {
+#pragma unroll
+      for (int m = 0; m < 8; ++m)
+        if (gx + m < gw) dst[m] = acc[m];
     }
   }
 }

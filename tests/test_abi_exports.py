@@ -7,10 +7,10 @@ import subprocess
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def declared_symbols():
-    text = open(os.path.join(ROOT, "include", "ffpp.h")).read()
+def declared_symbols(header="ffpp.h"):
+    text = open(os.path.join(ROOT, "include", header)).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(ffpp_[a-z_]+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b(ffpp_[a-z_0-9]+)\s*\(", text)))
 
 
 def test_library_builds_loads_and_exports_the_header():
@@ -19,7 +19,10 @@ def test_library_builds_loads_and_exports_the_header():
     lib = ctypes.CDLL(path)
     syms = declared_symbols()
     assert set(syms) == set(m.EXPORTS), (syms, m.EXPORTS)
-    for s in syms:
+    dbg = declared_symbols("ffpp_debug.h")
+    assert set(dbg) == set(m.DEBUG_EXPORTS), (dbg, m.DEBUG_EXPORTS)
+    assert not [s for s in syms if "debug" in s], "include/ffpp.h is the contract only"
+    for s in syms + dbg:
         assert hasattr(lib, s), f"libffpp.so does not export {s}"
     # null-handle calls that need no device
     lib.ffpp_destroy.argtypes = [ctypes.c_void_p]

@@ -182,7 +182,180 @@ def test_wild_box_sizes_against_every_threshold(env, thr):
     raw[twins, :4] = raw[twins[0], :4] * rng.uniform(0.97, 1.03, size=(300, 4))   # a pile of near-identical shapes
     raw[js, 4] = rng.uniform(-1.0, 8.0, size=3000)
     w = W(raw, [[640, 640]], dict(P, dtype="fp32", top_k=2500, iou_thresh=thr))
-    check(env, w, nms_edges_per_box=1300)               # room for every pair: at thr ~ 0 the frame-sized boxes touch everything
+    check(env, w)                                        # default pool: whatever does not fit goes through the overflow kernel
+    if thr in (0.0, 0.5):
+        check(env, w, nms_edges_per_box=1300)           # and with room for every pair (at thr ~ 0 the frame-sized boxes touch everything)
+
+
+def test_large_birds_on_the_finest_level_overflow_the_default_pool_and_still_match(env):
+    """A bird 120 px wide lights up ~120 stride-8 candidates that all regress (almost) the same box: ~60 suppression pairs
+    per box, far beyond the default 16 per top-K slot.  The frame must be bit-exact all the same."""
+    torch, m, oracle_mod, gen = env
+    rng = np.random.default_rng(21)
+    N = 8400
+    raw = frame(N, np.float16, rng, 0)
+    centres = rng.uniform(90.0, 550.0, size=(24, 2))
+    for cx, cy in centres:
+        for iy in range(80):
+            for ix in range(80):
+                px, py = (ix + 0.5) * 8, (iy + 0.5) * 8
+                if abs(px - cx) < 44 and abs(py - cy) < 44:
+                    j = iy * 80 + ix
+                    jit = rng.normal(0.0, 1.5, size=4)
+                    raw[j, :4] = (np.array([px - (cx - 60), py - (cy - 60), (cx + 60) - px, (cy + 60) - py]) + jit) / 8.0
+                    raw[j, 4] = rng.uniform(1.0, 6.0)
+    w = W(raw, [[640, 640]], dict(P, iou_thresh=0.5))
+    pp = m.FFPP.for_workload(w)
+    out = pp.run(torch.from_numpy(w.raw).cuda(), w.N_per_frame, w.frame_dims)
+    torch.cuda.synchronize()
+    assert pp.debug_read(5, 1)[0] == 1, "the case is meant to overflow the default pool"
+    compare(out, oracle_mod.run(w.params, w.raw, w.N_per_frame, w.frame_dims), w, check_stage=pp)
+
+
+def _iou32(a, b):
+    """numpy restatement of O5, op by op in fp32 — only used to CHOOSE cases; the expected result is the oracle's."""
+    f = np.float32
+    iw = max(f(0), f(min(a[2], b[2]) - max(a[0], b[0])))
+    ih = max(f(0), f(min(a[3], b[3]) - max(a[1], b[1])))
+    inter = f(iw * ih)
+    aa = f(f(a[2] - a[0]) * f(a[3] - a[1]))
+    ab = f(f(b[2] - b[0]) * f(b[3] - b[1]))
+    return f(inter / f(f(aa + ab) - inter))
+
+
+@pytest.mark.parametrize("thr", [float(np.float32(1.0) / np.float32(3.0)), 0.45, 0.5, 0.7])
+def test_pairs_at_and_around_the_iou_threshold(env, thr):
+    """Hand-built pairs whose fp32 IoU equals thr, is one ulp above / below it, and sits just inside / outside the
+    2^-20 guard band of iou_exceeds: the exact __fdiv_rn branch decides, as the oracle's division does.  One pair per
+    64x64 frame, coordinates below 32 px on a 2^-19 lattice so that one lattice step moves the IoU by ~2 ulps."""
+    torch, m, oracle_mod, gen = env
+    f32 = np.float32
+    t32 = f32(thr)
+    rng = np.random.default_rng(int(thr * 1000))
+    q = 2.0 ** -19
+    pairs = []
+    if abs(thr - 0.5) < 1e-9:
+        pairs.append((np.array([1, 2, 4, 3], f32), np.array([2, 2, 5, 3], f32)))        # inter 2, union 4: exactly 0.5
+    if abs(thr - 1 / 3) < 1e-6:
+        pairs.append((np.array([1, 2, 3, 3], f32), np.array([2, 2, 4, 3], f32)))        # inter 1, union 3: fl(1/3)
+    for _ in range(40):
+        wa, ha = np.round(rng.uniform(9, 14, 2) / q) * q
+        wb, hb = np.round(np.array([wa, ha]) * rng.uniform(0.9, 1.1, 2) / q) * q
+        A = np.array([2, 2, 2 + wa, 2 + ha], f32)
+        lo, hi = 0.0, float(wa)                        # B = A-sized box shifted right by d: IoU falls from ~1 to 0
+        for _ in range(60):
+            mid = np.round((lo + hi) / 2 / q) * q
+            Bx = np.array([2 + mid, 2, 2 + mid + wb, 2 + hb], f32)
+            if _iou32(A, Bx) > t32: lo = mid
+            else: hi = mid
+        for k in range(-6, 7):
+            d = lo + k * q
+            pairs.append((A, np.array([2 + d, 2, 2 + d + wb, 2 + hb], f32)))
+    ious = np.array([_iou32(a, b) for a, b in pairs], f32)
+    rel = np.abs(ious.astype(np.float64) - float(t32)) / float(t32)
+    assert (rel < 2.0 ** -20).sum() >= 20 and (ious > t32).any() and (ious <= t32).any()
+    assert (ious == t32).any() or (np.abs(ious.view(np.int32) - t32.view(np.int32)) <= 1).any(), "no pair within one ulp of thr"
+    dims, parts = [], []
+    for a, b in pairs:
+        fr = np.zeros((84, 5), np.float32); fr[:, :4] = 0.25; fr[:, 4] = -9.0
+        # A regressed from candidate (ix=1, iy=1): p = (12, 12); B from (ix=2, iy=1): p = (20, 12); stride 8
+        fr[9] = [(12 - a[0]) / 8, (12 - a[1]) / 8, (a[2] - 12) / 8, (a[3] - 12) / 8, 3.0]
+        fr[10] = [(20 - b[0]) / 8, (12 - b[1]) / 8, (b[2] - 20) / 8, (b[3] - 12) / 8, 2.0]
+        parts.append(fr); dims.append([64, 64])
+    w = W(np.concatenate(parts), dims, dict(P, dtype="fp32", iou_thresh=thr, top_k=16, sigma_cells=1.0))
+    out, ref = check(env, w)
+    dec = out.boxes_numpy()
+    for i, (a, b) in enumerate(pairs):                 # the decoded boxes ARE the intended ones, and the decision is the IoU's
+        assert np.array_equal(np.array(list(dec[i, 0])[:4], f32), a)
+        assert int(ref.counts[i]) == (1 if ious[i] > t32 else 2), (i, ious[i])
+
+
+def test_output_buffers_at_odd_offsets(env):
+    """out_density only needs 4-byte alignment (the float4 store path must look at the pointer, not only
+    at the offsets inside the batch); grids of 16-px and 32-px cells give per-frame sizes that are not multiples of 4."""
+    torch, m, oracle_mod, gen = env
+    rng = np.random.default_rng(31)
+    dims = [[160, 96], [224, 96], [640, 640], [160, 96]]
+    for cell, sig in ((32, 1.0), (16, 1.0), (8, 2.0)):
+        parts = [frame(gen.frame_candidates(a, b), np.float16, rng, 40, lo=0.0, hi=8.0) for a, b in dims]
+        w = W(np.concatenate(parts), dims, dict(P, cell_px=cell, sigma_cells=sig, truncate_sigmas=1.0 if cell == 32 else 3.0))
+        pp = m.FFPP.for_workload(w)
+        ref = oracle_mod.run(w.params, w.raw, w.N_per_frame, w.frame_dims)
+        for shift in (0, 1, 2, 3):
+            out = pp.alloc_outputs(len(dims), w.frame_dims)
+            cells = int(out.density_offsets[-1])
+            big = torch.full((cells + 8,), -1.0, dtype=torch.float32, device="cuda")
+            out.density = big[shift:shift + cells]
+            pp.run(torch.from_numpy(w.raw).cuda(), w.N_per_frame, w.frame_dims, out=out)
+            torch.cuda.synchronize()
+            compare(out, ref, w)
+            assert (big[:shift] == -1).all() and (big[shift + cells:] == -1).all()
+
+
+def test_cuda_graph_capture_and_replay(env):
+    """include/ffpp.h: ffpp_run is capturable once the batch geometry is cached.  Capture one run, replay it on
+    NEW inputs written into the same buffers, compare with the oracle; an uncached geometry under capture is refused."""
+    torch, m, oracle_mod, gen = env
+    w0 = gen.make_config(5, B=8, seed_offset=3)
+    w1 = gen.make_config(5, B=8, seed_offset=4)
+    pp = m.FFPP.for_workload(w0)
+    raw = torch.from_numpy(w0.raw).cuda()
+    out = pp.alloc_outputs(w0.B, w0.frame_dims)
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        pp.run(raw, w0.N_per_frame, w0.frame_dims, out=out)          # caches the geometry
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        pp.run(raw, w0.N_per_frame, w0.frame_dims, out=out)
+    out.counts.zero_(); out.density.zero_()
+    g.replay(); torch.cuda.synchronize()
+    compare(out, oracle_mod.run(w0.params, w0.raw, w0.N_per_frame, w0.frame_dims), w0)
+    raw.copy_(torch.from_numpy(w1.raw))
+    for _ in range(2):
+        g.replay()
+    torch.cuda.synchronize()
+    compare(out, oracle_mod.run(w1.params, w1.raw, w1.N_per_frame, w1.frame_dims), w1)
+    # a geometry the handle has not seen cannot be captured (its descriptor upload reads host memory)
+    w2 = gen.make_config(5, B=4, seed_offset=3)
+    raw2 = torch.from_numpy(w2.raw).cuda()
+    out2 = pp.alloc_outputs(w2.B, w2.frame_dims)
+    g2 = torch.cuda.CUDAGraph()
+    with pytest.raises(m.FFPPError) as ei:
+        with torch.cuda.graph(g2):
+            pp.run(raw2, w2.N_per_frame, w2.frame_dims, out=out2)
+    assert ei.value.code == m.FFPP_EINVAL and "capture" in str(ei.value)
+    torch.cuda.synchronize()
+
+
+def test_alternating_geometries_never_wait_for_the_device(env):
+    """ffpp_run never synchronises the host.  With ~0.3 s of spinning queued ahead on the stream, calls with
+    a cached geometry, a NEW geometry and the first one again must all return while the spin is still running."""
+    import time
+    torch, m, oracle_mod, gen = env
+    wa = gen.make_config(5, B=4)
+    wb = gen.make_config(5, B=3, seed_offset=1)
+    wc = gen.make_config(5, B=6, seed_offset=2)
+    big = gen.make_config(5, B=8)
+    pp = m.FFPP.for_workload(big)
+    ra, rb, rc = (torch.from_numpy(x.raw).cuda() for x in (wa, wb, wc))
+    oa = pp.run(ra, wa.N_per_frame, wa.frame_dims)
+    torch.cuda.synchronize()
+    st = torch.cuda.current_stream()
+    torch.cuda._sleep(int(0.3 * 1.9e9))
+    t0 = time.perf_counter()
+    oa = pp.run(ra, wa.N_per_frame, wa.frame_dims)
+    ob = pp.run(rb, wb.N_per_frame, wb.frame_dims)               # new geometry: descriptor build + stream-ordered upload
+    oc = pp.run(rc, wc.N_per_frame, wc.frame_dims)               # another new one
+    oa2 = pp.run(ra, wa.N_per_frame, wa.frame_dims)
+    dt = time.perf_counter() - t0
+    still_running = not st.query()
+    torch.cuda.synchronize()
+    assert still_running and dt < 0.1, f"ffpp_run blocked the host: {dt:.3f} s, spin still running: {still_running}"
+    for o, x in ((oa2, wa), (ob, wb), (oc, wc)):
+        compare(o, oracle_mod.run(x.params, x.raw, x.N_per_frame, x.frame_dims), x)
 
 
 @pytest.mark.parametrize("sigma,trunc,R", [(0.5, 3.0, 1), (1.0, 3.0, 3), (1.7, 3.0, 5), (3.7, 3.0, 11), (4.4, 3.0, 13),
