@@ -57,7 +57,6 @@ struct ffpp_handle {
   int* d_counters = nullptr;          // 4 x max_frames: survivor counts | top-K counts | edge counters | frame_err
   float4* d_sel_box = nullptr;        // a2 scratch: decoded boxes in selection order; 
   float4* d_sp_box = nullptr;         // boxes in spatial order (row-major 16-px cell of the centre), stride kpad per frame
-  float4* d_sp_sbox = nullptr;        // culling boxes
   void* d_sp_key = nullptr;
   uint8_t* d_hasin = nullptr;         // a3 -> a4: one byte per box, 1 = victim of at least one edge
   void* d_kept_key = nullptr;         // a4: keys of the kept boxes in keep order, top_k per frame
@@ -261,7 +260,7 @@ int launch_all(ffpp_handle* h, const void* raw, int B, cudaStream_t st, ffpp_box
   // a2 (+ clears the a5 histogram)
   k2_select_bin<kHalf, KeyT><<<B, K2_THREADS, k2_smem_bytes((size_t)c.top_k, sizeof(KeyT)), st>>>(
       static_cast<const uint8_t*>(raw), frames, static_cast<const KeyT*>(h->d_surv_keys), h->surv_cnt(), c,
-      h->d_sel_box, h->d_sp_box, h->d_sp_sbox, static_cast<KeyT*>(h->d_sp_key), h->d_cellstart, h->n_sorted(), h->d_hist32,
+      h->d_sel_box, h->d_sp_box, static_cast<KeyT*>(h->d_sp_key), h->d_cellstart, h->n_sorted(), h->d_hist32,
       reinterpret_cast<uint32_t*>(h->d_hasin), h->sm_count);
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[3], st));
   // a3 (+ the pool-free overflow path: its CTAs exit at once unless k3 flagged their frame)
@@ -269,14 +268,14 @@ int launch_all(ffpp_handle* h, const void* raw, int B, cudaStream_t st, ffpp_box
     const dim3 g3((unsigned)((g.max_nmax + K3_THREADS - 1) / K3_THREADS), (unsigned)B);
     if (g3.x > 0) {
       if (h->count_work)
-        k3_nms_edges<KeyT, true><<<g3, K3_THREADS, 0, st>>>(frames, h->n_sorted(), h->d_sp_box, h->d_sp_sbox,
+        k3_nms_edges<KeyT, true><<<g3, K3_THREADS, 0, st>>>(frames, h->n_sorted(), h->d_sp_box,
                                                             static_cast<const KeyT*>(h->d_sp_key), h->d_cellstart, c,
                                                             h->edge_ctr(), h->d_edges, h->d_hasin, h->frame_err(), h->d_work);
       else
-        k3_nms_edges<KeyT, false><<<g3, K3_THREADS, 0, st>>>(frames, h->n_sorted(), h->d_sp_box, h->d_sp_sbox,
+        k3_nms_edges<KeyT, false><<<g3, K3_THREADS, 0, st>>>(frames, h->n_sorted(), h->d_sp_box,
                                                              static_cast<const KeyT*>(h->d_sp_key), h->d_cellstart, c,
                                                              h->edge_ctr(), h->d_edges, h->d_hasin, h->frame_err(), h->d_work);
-      k3o_overflow<KeyT><<<B, K3O_THREADS, (size_t)c.kpad, st>>>(frames, h->n_sorted(), h->d_sp_box, h->d_sp_sbox,
+      k3o_overflow<KeyT><<<B, K3O_THREADS, (size_t)c.kpad, st>>>(frames, h->n_sorted(), h->d_sp_box,
                                                                 static_cast<const KeyT*>(h->d_sp_key), h->d_cellstart, c,
                                                                 h->edge_ctr(), h->d_hasin, h->frame_err());
     }
@@ -377,7 +376,6 @@ int ffpp_create(const ffpp_params* p, ffpp_handle** out) {
   c.iou_fast = (p->iou_thresh >= 1e-6f && p->iou_thresh <= 1e6f) ? 1 : 0;
   c.iou_thr_hi = std::nextafterf((float)((double)p->iou_thresh * (1.0 + std::ldexp(1.0, -20))), INFINITY);
   c.iou_thr_lo = std::nextafterf((float)((double)p->iou_thresh * (1.0 - std::ldexp(1.0, -20))), -INFINITY);
-  c.shrink = (p->iou_thresh >= 0.05f) ? 0.49f * std::min(p->iou_thresh, 1.0f) : 0.0f;
   {
     // a pair with IoU > t has |centre distance| < rho * min(w_a, w_b) per axis, rho = max(1 - t, 1/(2t) - 1/2); evaluated
     // at a slightly smaller t (and at most 0.9) so that every fp32 rounding of the IoU of the definition is covered
@@ -437,7 +435,6 @@ int ffpp_create(const ffpp_params* p, ffpp_handle** out) {
       (e = dalloc((void**)&h->d_counters, (3 + kCntStride) * F * sizeof(int))) != cudaSuccess ||
       (e = dalloc((void**)&h->d_sel_box, F * KP * sizeof(float4))) != cudaSuccess ||
       (e = dalloc((void**)&h->d_sp_box, F * KP * sizeof(float4))) != cudaSuccess ||
-      (e = dalloc((void**)&h->d_sp_sbox, F * KP * sizeof(float4))) != cudaSuccess ||
       (e = dalloc(&h->d_sp_key, F * KP * (size_t)h->key_bytes)) != cudaSuccess ||
       (e = dalloc((void**)&h->d_hasin, F * KP)) != cudaSuccess ||
       (e = dalloc(&h->d_kept_key, F * (size_t)p->top_k * (size_t)h->key_bytes)) != cudaSuccess ||
@@ -630,7 +627,7 @@ int ffpp_destroy(ffpp_handle* h) {
   if (!h) return FFPP_OK;
   for (int sl = 0; sl < ffpp_handle::kGeoSlots; ++sl) cudaFree(h->geo[sl].d_meta);
   cudaFree(h->d_work); cudaFree(h->d_surv_keys); cudaFree(h->d_counters); cudaFree(h->d_sel_box); cudaFree(h->d_sp_box);
-  cudaFree(h->d_sp_sbox); cudaFree(h->d_sp_key); cudaFree(h->d_cellstart); cudaFree(h->d_hasin); cudaFree(h->d_k4_scratch); cudaFree(h->d_kept_key); cudaFree(h->d_kept_pos); cudaFree(h->d_edges);
+  cudaFree(h->d_sp_key); cudaFree(h->d_cellstart); cudaFree(h->d_hasin); cudaFree(h->d_k4_scratch); cudaFree(h->d_kept_key); cudaFree(h->d_kept_pos); cudaFree(h->d_edges);
   cudaFree(h->d_hist32);
   cudaFree(h->d_in); cudaFree(h->d_out_boxes); cudaFree(h->d_out_counts); cudaFree(h->d_out_density);
   if (h->s_h2d) cudaStreamDestroy(h->s_h2d);

@@ -39,7 +39,6 @@ struct Consts {
   float logit_thr;                  // T
   float iou_thr, iou_thr_hi, iou_thr_lo;
   int32_t iou_fast;                 // 1: the guard-banded multiply test is valid for this threshold
-  float shrink;                     // per-side shrink factor of the culling boxes: 0.49 * min(iou_thr, 1), or 0
   float rho;                        // partner-centre window half-extent in units of the box's own width/height (a3)
   int32_t top_k;
   int32_t kpad;                     // top_k rounded up to a multiple of 32: per-frame stride of the spatial arrays
@@ -90,19 +89,6 @@ template <typename KeyT> __device__ __forceinline__ int idx_of_key(KeyT key) {
 }
 template <typename KeyT> __device__ __forceinline__ float logit_of_key(KeyT key) {
   return sizeof(KeyT) == 4 ? logit_of_key16((uint32_t)key >> 16) : logit_of_key32((uint32_t)((uint64_t)key >> 32));
-}
-
-// ---- culling box (DESIGN.md §6 a3) ----
-// IoU(a,b) > t implies iw > t*max(wa,wb) >= t*(wa+wb)/2 (inter = iw*ih > t*union >= t*wa*ha and ih <= ha), i.e. the boxes
-// still overlap, strictly, after each is shrunk by t/2 of its width (height) per side.  The culling boxes use
-// 0.49*t instead of 0.5*t: the 2 % slack dwarfs every fp32 rounding in this function and in the fp32 IoU of the
-// definition as long as the box is not tiny against its coordinates, which the w > 1e-3*(|x1|+|x2|) test ensures
-// (otherwise, and for NaN/inf/inverted boxes, that axis is left unshrunk, which is always conservative).
-__device__ __forceinline__ float4 shrink_box(const float4 b, const float c) {
-  const float w = __fsub_rn(b.z, b.x), h = __fsub_rn(b.w, b.y);
-  const float dx = (w > 1e-3f * (fabsf(b.x) + fabsf(b.z))) ? __fmul_rn(c, w) : 0.0f;
-  const float dy = (h > 1e-3f * (fabsf(b.y) + fabsf(b.w))) ? __fmul_rn(c, h) : 0.0f;
-  return make_float4(__fadd_rn(b.x, dx), __fadd_rn(b.y, dy), __fsub_rn(b.z, dx), __fsub_rn(b.w, dy));
 }
 
 // ---- spatial cells (a2 bins with these, a3 builds its windows with these: the same two functions on both sides) ----

@@ -253,7 +253,7 @@ __device__ __forceinline__ int blk_scan_inclusive(int v, BlkMisc* misc, int par,
 //  (3) decode the selected rows from the raw head output (fp32, cell-centre grid point, no clipping; O1, O2) and bin
 //      each box by the spatial cell of its centre (row-major cells of 2^hshift pixels, <= 16384 per frame) with one
 //      shared atomic (counting sort);
-//  (4) scan the bins, scatter box / culling box / key to the frame's spatial arrays, and write the cell-start table
+//  (4) scan the bins, scatter box / key to the frame's spatial arrays, and write the cell-start table
 //      (uint16 start position of every cell, row-major) that a3 uses to enumerate the boxes of a window of cells.
 // The (score desc, index asc) ORDER itself is applied where it is consumed: as key comparisons in a3/a4 (greedy NMS
 // only ever asks "which of two boxes comes first") and as a radix sort of the kept keys in a4, which is ~8x fewer
@@ -273,7 +273,7 @@ template <bool kHalf, typename KeyT>
 __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
     const uint8_t* __restrict__ raw, const FrameDesc* __restrict__ frames, const KeyT* __restrict__ surv_keys,
     const int* __restrict__ surv_cnt, Consts cst, float4* __restrict__ sel_box, float4* __restrict__ sp_box,
-    float4* __restrict__ sp_sbox, KeyT* __restrict__ sp_key, uint16_t* __restrict__ cellstart,
+    KeyT* __restrict__ sp_key, uint16_t* __restrict__ cellstart,
     int* __restrict__ n_sorted, uint32_t* __restrict__ hist32, uint32_t* __restrict__ hasin, int sm_count) {
   constexpr int KB = sizeof(KeyT) * 8;
   extern __shared__ __align__(16) uint8_t smem[];
@@ -489,7 +489,6 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
         const uint32_t a = aux[i];
         const int pos = (int)base16[a >> 16] + (int)(a & 0xFFFFu);
         sp_box[obase + pos] = box[u];
-        sp_sbox[obase + pos] = shrink_box(box[u], cst.shrink);
         sp_key[obase + pos] = sel[i];
       }
     }
@@ -512,28 +511,32 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
 // which bits are ever looked at.  Boxes are sorted by the row-major spatial cell of their centre (a2).  A pair with
 // IoU > thr has, on each axis, |centre_a - centre_b| < rho * min(w_a, w_b)  (from iw > thr * max(w_a, w_b) and
 // |dc| <= (w_a + w_b)/2 - iw;  rho = max(1 - thr, 1/(2 thr) - 1/2), DESIGN.md §6 a3), so the partner of box a lies
-// in a window of cells around a's own cell that a computes from its own size.  One thread per box; every unordered
-// pair is examined once, by the member that comes first in the spatial order: it scans the rest of its own cell row
-// and the window's rows below, each row one contiguous range of the sorted arrays, through the cell-start table.
-//  (1) pretest on the culling boxes (boxes shrunk by ~thr/2 per side, see shrink_box): 4 compares per candidate,
-//      two candidates per thread per step, all 32 threads of a warp stepping together;
-//  (2) the surviving (row, candidate) pairs are ballot-compacted into a per-warp queue and evaluated 32 at a time,
-//      one pair per lane, with the fp32 IoU of the definition (iou_exceeds) — full lanes on the expensive part;
-//  (3) a hit becomes the edge (victim << 16 | suppressor), spatial positions, the suppressor being the member that
-//      comes first in the order of O4 (smaller key); edges are staged per warp and appended to the frame's edge pool
-//      with one atomicAdd per flush, and the victim's "has a suppressor" byte is set (a plain store).
+// in a window of cells around a's own cell that a computes from its own size.  Every unordered pair is examined once,
+// by the member that comes first in the spatial order: its candidates are the rest of its own cell row and the
+// window's rows below, each row one contiguous range of the sorted arrays, found through the cell-start table.
+// A warp owns 32 consecutive boxes and works in two alternating phases, so that the expensive part runs on full lanes
+// whatever the shape of the individual windows:
+//  (1) fill: every lane appends its (owner lane, candidate position) pairs of one window row to the warp's work list
+//      in shared memory (warp prefix sum of the range lengths; a short divergent loop of 3 instructions per entry);
+//  (2) drain: the list is consumed 32 entries at a time, one pair per lane: the owner's box comes from shared memory,
+//      the candidate's from the sorted array, and the fp32 IoU of the definition (iou_exceeds) decides.  A hit becomes
+//      the edge (victim << 16 | suppressor), spatial positions, the suppressor being the member that comes first in
+//      the order of O4 (smaller key); edges are staged per warp and appended to the frame's edge pool with one
+//      atomicAdd per flush, and the victim's "has a suppressor" byte is set (a plain store).
+// The list is drained only when it is full or the warp has no rows left, so all but the last step of a warp are full.
 // =====================================================================================================
-constexpr uint32_t ST_U = 0, ST_K = 1, ST_R = 2;   // box state of the greedy fixed point (a3 overflow path, a4)
+constexpr uint32_t ST_U = 0, ST_K = 1, ST_R = 2;   // box state of the greedy fixed point (overflow path, a4)
 constexpr int K3_WARPS = 8;
 constexpr int K3_THREADS = 32 * K3_WARPS;
-constexpr int K3_QCAP = 96;                     // candidate queue: <= 31 left over + <= 64 pushed per step
+constexpr int K3_CHUNK = 32;                    // entries one lane appends per fill step
+constexpr int K3_LCAP = 32 * K3_CHUNK + 32;     // work list: one full fill step on top of a < 32 entry remainder
 constexpr int K3_SCAP = 128;                    // edge staging per warp
 
 template <typename KeyT>
 struct K3Warp {
   float4 rowbox[32];
   KeyT rowkey[32];
-  uint32_t q[K3_QCAP];
+  uint32_t list[K3_LCAP];
   uint32_t sb[K3_SCAP];
 };
 
@@ -541,14 +544,13 @@ template <typename KeyT, bool kCount>
 __global__ void __launch_bounds__(K3_THREADS) k3_nms_edges(const FrameDesc* __restrict__ frames,
                                                            const int* __restrict__ n_sorted,
                                                            const float4* __restrict__ sp_box,
-                                                           const float4* __restrict__ sp_sbox,
                                                            const KeyT* __restrict__ sp_key,
                                                            const uint16_t* __restrict__ cellstart, Consts cst,
                                                            int* __restrict__ edge_ctr, uint32_t* __restrict__ edges,
                                                            uint8_t* __restrict__ hasin, int* __restrict__ frame_err,
                                                            unsigned long long* __restrict__ work_ctr) {
   __shared__ K3Warp<KeyT> s_w[K3_WARPS];
-  unsigned long long n_pre = 0, n_exact = 0, n_edge = 0;      // kCount only: this lane's culling tests / IoUs / edges
+  unsigned long long n_exact = 0, n_edge = 0;                 // kCount only: this lane's exact IoUs / edges
 
   const int f = blockIdx.y;
   const int n = n_sorted[f];
@@ -556,12 +558,11 @@ __global__ void __launch_bounds__(K3_THREADS) k3_nms_edges(const FrameDesc* __re
   if (p0 >= n) return;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   if (p0 + warp * 32 >= n) return;
-  if (!kCount && *reinterpret_cast<volatile int*>(&frame_err[f])) return;   // the frame already goes to k3o_overflow
+  if (!kCount && *reinterpret_cast<volatile int*>(&frame_err[f])) return;   // the frame already goes to the overflow path
   const FrameDesc* fd = &frames[f];
   const int cgw = fd->cgw, cgh = fd->cgh, hs = fd->hshift;
   const int64_t obase = (int64_t)f * cst.kpad;
   const float4* fbox = sp_box + obase;
-  const float4* fsbox = sp_sbox + obase;
   const KeyT* fkey = sp_key + obase;
   const uint16_t* cs = cellstart + (int64_t)f * kCellStride;
   K3Warp<KeyT>& W = s_w[warp];
@@ -572,7 +573,6 @@ __global__ void __launch_bounds__(K3_THREADS) k3_nms_edges(const FrameDesc* __re
   const bool valid = p < n;
   const int pc = valid ? p : n - 1;
   const float4 a = fbox[pc];
-  const float4 sa = fsbox[pc];
   W.rowbox[lane] = a;
   W.rowkey[lane] = fkey[pc];
 
@@ -583,11 +583,8 @@ __global__ void __launch_bounds__(K3_THREADS) k3_nms_edges(const FrameDesc* __re
   const float ey = fmaxf(cst.rho * (a.w - a.y), 0.0f) * 1.001f + 1e-5f * (fabsf(a.y) + fabsf(a.w));
   const int Xlo = cell_coord(cxa - ex, cmx, hs), Xhi = cell_coord(cxa + ex, cmx, hs);
   const int Ya = cell_coord(cya, cmy, hs);
-  int Yhi = cell_coord(cya + ey, cmy, hs);
-
-  int Y = Ya, j = p + 1, e = cs[Ya * cgw + Xhi + 1];
-  if (!valid) { Y = Yhi = 0; j = e = 0; }
-  int qcnt = 0, scnt = 0;                          // warp-uniform
+  const int Yhi = cell_coord(cya + ey, cmy, hs);
+  int lcnt = 0, scnt = 0;                          // warp-uniform
   __syncwarp();
 
   auto flush = [&]() {
@@ -598,17 +595,17 @@ __global__ void __launch_bounds__(K3_THREADS) k3_nms_edges(const FrameDesc* __re
     if (base + scnt <= fd->edge_cap) {
       for (int k = lane; k < scnt; k += 32) edges[fd->edge_off + base + k] = W.sb[k];
     } else if (lane == 0) {
-      frame_err[f] = 1;                            // the frame's pool share is exhausted: k3o_overflow resolves the frame
+      frame_err[f] = 1;                            // the frame's pool share is exhausted: the overflow path resolves the frame
     }
     scnt = 0;
     __syncwarp();
   };
-  // evaluate `nb` (<= 32) queued candidates, one per lane, from the top of the queue
-  auto exact_batch = [&](const int nb) {
+  // evaluate entries [i0, i0 + nb) of the work list, one per lane
+  auto exact_step = [&](const int i0, const int nb) {
     bool hit = false;
     uint32_t ed = 0;
     if (lane < nb) {
-      const uint32_t q = W.q[qcnt - nb + lane];
+      const uint32_t q = W.list[i0 + lane];
       const uint32_t al = q >> 16, b = q & 0xFFFFu;
       if (kCount) ++n_exact;
       if (iou_exceeds(W.rowbox[al], fbox[b], cst)) {
@@ -622,45 +619,53 @@ __global__ void __launch_bounds__(K3_THREADS) k3_nms_edges(const FrameDesc* __re
     const uint32_t bal = __ballot_sync(0xffffffffu, hit);
     if (hit) W.sb[scnt + __popc(bal & lt)] = ed;
     scnt += __popc(bal);
-    qcnt -= nb;
     __syncwarp();
     if (scnt > K3_SCAP - 32) flush();
   };
-
-  for (;;) {
-    while (j >= e && Y < Yhi) {
-      ++Y;
-      const uint16_t* r = cs + Y * cgw;
-      j = r[Xlo];
-      e = r[Xhi + 1];
-    }
-    const bool act = j < e;
-    if (!__any_sync(0xffffffffu, act)) break;
-    bool h0 = false, h1 = false;
-    if (act) {
-      const bool two = j + 1 < e;
-      const float4 sb0 = fsbox[j];
-      const float4 sb1 = fsbox[two ? j + 1 : j];
-      h0 = boxes_overlap(sa, sb0);
-      h1 = two && boxes_overlap(sa, sb1);
-      if (kCount) n_pre += two ? 2 : 1;
-    }
-    const uint32_t b0 = __ballot_sync(0xffffffffu, h0), b1 = __ballot_sync(0xffffffffu, h1);
-    if (b0 | b1) {
-      const int c0 = __popc(b0);
-      if (h0) W.q[qcnt + __popc(b0 & lt)] = ((uint32_t)lane << 16) | (uint32_t)j;
-      if (h1) W.q[qcnt + c0 + __popc(b1 & lt)] = ((uint32_t)lane << 16) | (uint32_t)(j + 1);
-      qcnt += c0 + __popc(b1);
+  // consume the full 32-entry steps of the list; the remainder (< 32 entries) moves to the front, or is evaluated too
+  auto drain = [&](const bool all) {
+    int i = 0;
+    for (; i + 32 <= lcnt; i += 32) exact_step(i, 32);
+    const int rem = lcnt - i;
+    if (rem > 0 && all) { exact_step(i, rem); lcnt = 0; return; }
+    if (rem > 0 && i > 0) {
+      const uint32_t v = lane < rem ? W.list[i + lane] : 0u;
       __syncwarp();
-      while (qcnt >= 32) exact_batch(32);
+      if (lane < rem) W.list[lane] = v;
+      __syncwarp();
     }
-    j += 2;
+    lcnt = rem;
+  };
+
+  for (int rr = 0;; ++rr) {
+    const int Y = Ya + rr;
+    const bool act = valid && Y <= Yhi;
+    if (!__any_sync(0xffffffffu, act)) break;
+    int j = 0, rem = 0;
+    if (act) {
+      const uint16_t* r = cs + Y * cgw;
+      j = rr == 0 ? p + 1 : (int)r[Xlo];
+      rem = max((int)r[Xhi + 1] - j, 0);
+    }
+    while (__any_sync(0xffffffffu, rem > 0)) {
+      const int c = min(rem, K3_CHUNK);
+      int inc = c;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
+      const int total = __shfl_sync(0xffffffffu, inc, 31);
+      if (lcnt + total > K3_LCAP) drain(false);    // leaves < 32 entries: a whole fill step fits
+      uint32_t* dst = W.list + lcnt + inc - c;
+      const uint32_t e0 = ((uint32_t)lane << 16) | (uint32_t)j;
+      for (int i = 0; i < c; ++i) dst[i] = e0 + (uint32_t)i;
+      j += c; rem -= c; lcnt += total;
+      __syncwarp();
+    }
   }
-  if (qcnt > 0) exact_batch(qcnt);
+  drain(true);
   flush();
   if (kCount) {
-    n_pre = warp_sum_u64(n_pre); n_exact = warp_sum_u64(n_exact); n_edge = warp_sum_u64(n_edge);
-    if (lane == 0) { atomicAdd(&work_ctr[0], n_pre); atomicAdd(&work_ctr[1], n_exact); atomicAdd(&work_ctr[2], n_edge); }
+    n_exact = warp_sum_u64(n_exact); n_edge = warp_sum_u64(n_edge);
+    if (lane == 0) { atomicAdd(&work_ctr[1], n_exact); atomicAdd(&work_ctr[2], n_edge); }
   }
 }
 
@@ -668,8 +673,8 @@ __global__ void __launch_bounds__(K3_THREADS) k3_nms_edges(const FrameDesc* __re
 // a3/a4 overflow path — a frame whose suppression pairs do not fit its share of the edge pool (k3 raised frame_err[f]).
 // Greedy NMS is the unique fixed point of  kept(a) <=> no kept b before a with IoU(a,b) > thr;  this kernel iterates to
 // it WITHOUT storing pairs: one CTA per flagged frame (all other CTAs exit at once), one state byte per box in shared
-// memory, and per round every undecided box re-examines its partner window (the same cell window and culling-box
-// pretest as k3, both directions this time):
+// memory, and per round every undecided box re-examines its partner window (the same cell window as k3, both
+// directions this time):
 //     some kept partner before it has IoU > thr          -> removed
 //     no undecided-or-kept partner before it has IoU > thr -> kept
 //     otherwise                                             -> stays undecided.
@@ -681,7 +686,7 @@ __global__ void __launch_bounds__(K3_THREADS) k3_nms_edges(const FrameDesc* __re
 constexpr int K3O_THREADS = 1024;
 template <typename KeyT>
 __global__ void __launch_bounds__(K3O_THREADS) k3o_overflow(const FrameDesc* __restrict__ frames, const int* __restrict__ n_sorted,
-                                                            const float4* __restrict__ sp_box, const float4* __restrict__ sp_sbox,
+                                                            const float4* __restrict__ sp_box,
                                                             const KeyT* __restrict__ sp_key, const uint16_t* __restrict__ cellstart,
                                                             Consts cst, int* __restrict__ edge_ctr, uint8_t* __restrict__ hasin,
                                                             const int* __restrict__ frame_err) {
@@ -694,7 +699,6 @@ __global__ void __launch_bounds__(K3O_THREADS) k3o_overflow(const FrameDesc* __r
   const int cgw = fd->cgw, cgh = fd->cgh, hs = fd->hshift;
   const int64_t obase = (int64_t)f * cst.kpad;
   const float4* fbox = sp_box + obase;
-  const float4* fsbox = sp_sbox + obase;
   const KeyT* fkey = sp_key + obase;
   const uint16_t* cs = cellstart + (int64_t)f * kCellStride;
   volatile uint8_t* st = s_state;
@@ -706,7 +710,6 @@ __global__ void __launch_bounds__(K3O_THREADS) k3o_overflow(const FrameDesc* __r
     for (int p = tid; p < n; p += K3O_THREADS) {
       if (st[p] != ST_U) continue;
       const float4 a = fbox[p];
-      const float4 sa = fsbox[p];
       const KeyT ka = fkey[p];
       const float cxa = box_centre(a.x, a.z), cya = box_centre(a.y, a.w);
       const float ex = fmaxf(cst.rho * (a.z - a.x), 0.0f) * 1.001f + 1e-5f * (fabsf(a.x) + fabsf(a.z));
@@ -721,8 +724,9 @@ __global__ void __launch_bounds__(K3O_THREADS) k3o_overflow(const FrameDesc* __r
           const uint32_t sj = st[j];
           if (sj == ST_R || j == p) continue;
           if (!(fkey[j] < ka)) continue;                       // only a box BEFORE a in the order of O4 can suppress it
-          if (!boxes_overlap(sa, fsbox[j])) continue;
-          if (!iou_exceeds(a, fbox[j], cst)) continue;
+          const float4 b = fbox[j];
+          if (!boxes_overlap(a, b)) continue;                  // inter == 0: IoU > thr is false for every thr >= 0
+          if (!iou_exceeds(a, b, cst)) continue;
           if (sj == ST_K) { removed = true; break; }
           blocked = true;
         }
