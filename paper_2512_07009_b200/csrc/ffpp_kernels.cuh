@@ -526,11 +526,11 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
 // The list is drained only when it is full or the warp has no rows left, so all but the last step of a warp are full.
 // =====================================================================================================
 constexpr uint32_t ST_U = 0, ST_K = 1, ST_R = 2;   // box state of the greedy fixed point (overflow path, a4)
-constexpr int K3_WARPS = 8;
+constexpr int K3_WARPS = 4;
 constexpr int K3_THREADS = 32 * K3_WARPS;
-constexpr int K3_CHUNK = 32;                    // entries one lane appends per fill step
+constexpr int K3_CHUNK = 16;                    // entries one lane appends per fill step
 constexpr int K3_LCAP = 32 * K3_CHUNK + 32;     // work list: one full fill step on top of a < 32 entry remainder
-constexpr int K3_SCAP = 128;                    // edge staging per warp
+constexpr int K3_SCAP = 256;                    // hit staging per warp (a warp of the flock workloads has ~200)
 
 template <typename KeyT>
 struct K3Warp {
@@ -541,7 +541,7 @@ struct K3Warp {
 };
 
 template <typename KeyT, bool kCount>
-__global__ void __launch_bounds__(K3_THREADS) k3_nms_edges(const FrameDesc* __restrict__ frames,
+__global__ void __launch_bounds__(K3_THREADS, 12) k3_nms_edges(const FrameDesc* __restrict__ frames,
                                                            const int* __restrict__ n_sorted,
                                                            const float4* __restrict__ sp_box,
                                                            const KeyT* __restrict__ sp_key,
@@ -587,47 +587,71 @@ __global__ void __launch_bounds__(K3_THREADS) k3_nms_edges(const FrameDesc* __re
   int lcnt = 0, scnt = 0;                          // warp-uniform
   __syncwarp();
 
+  // staged hits are (owner lane << 16 | candidate position); the flush turns them into edges on full lanes: the
+  // suppressor is the member that comes first in the order of O4 (smaller key), the victim's flag byte is set
+  const int edge_cap = fd->edge_cap;
+  uint32_t* const fedges = edges + fd->edge_off;
+  uint8_t* const fhas = hasin + obase;
   auto flush = [&]() {
     if (scnt == 0) return;
+    __syncwarp();
     int base = 0;
     if (lane == 0) base = atomicAdd(&edge_ctr[f], scnt);
     base = __shfl_sync(0xffffffffu, base, 0);
-    if (base + scnt <= fd->edge_cap) {
-      for (int k = lane; k < scnt; k += 32) edges[fd->edge_off + base + k] = W.sb[k];
+    if (base + scnt <= edge_cap) {
+      for (int k = lane; k < scnt; k += 32) {
+        const uint32_t q = W.sb[k];
+        const uint32_t al = q >> 16, b = q & 0xFFFFu, pa = (uint32_t)row0 + al;
+        const uint32_t ed = fkey[b] < W.rowkey[al] ? ((pa << 16) | b) : ((b << 16) | pa);
+        fhas[ed >> 16] = 1;                        // a4 starts every box that is nobody's victim as kept
+        fedges[base + k] = ed;
+      }
     } else if (lane == 0) {
       frame_err[f] = 1;                            // the frame's pool share is exhausted: the overflow path resolves the frame
     }
     scnt = 0;
     __syncwarp();
   };
-  // evaluate entries [i0, i0 + nb) of the work list, one per lane
-  auto exact_step = [&](const int i0, const int nb) {
-    bool hit = false;
-    uint32_t ed = 0;
-    if (lane < nb) {
-      const uint32_t q = W.list[i0 + lane];
-      const uint32_t al = q >> 16, b = q & 0xFFFFu;
-      if (kCount) ++n_exact;
-      if (iou_exceeds(W.rowbox[al], fbox[b], cst)) {
-        hit = true;
-        if (kCount) ++n_edge;
-        const uint32_t pa = (uint32_t)row0 + al;
-        ed = fkey[b] < W.rowkey[al] ? ((pa << 16) | b) : ((b << 16) | pa);
-        hasin[obase + (ed >> 16)] = 1;             // a4 starts every box that is nobody's victim as kept
-      }
-    }
+  // record the hits of one step (one pair per lane) in the staging area
+  auto stage_hits = [&](const bool hit, const uint32_t q) {
     const uint32_t bal = __ballot_sync(0xffffffffu, hit);
-    if (hit) W.sb[scnt + __popc(bal & lt)] = ed;
+    if (hit) W.sb[scnt + __popc(bal & lt)] = q;
     scnt += __popc(bal);
-    __syncwarp();
     if (scnt > K3_SCAP - 32) flush();
   };
-  // consume the full 32-entry steps of the list; the remainder (< 32 entries) moves to the front, or is evaluated too
+  // consume the full 32-entry steps of the list, one pair per lane per step, the next step's entry and candidate box
+  // already in flight while this step's IoU is evaluated; the remainder (< 32 entries) moves to the front, or is
+  // evaluated too (`all`)
   auto drain = [&](const bool all) {
     int i = 0;
-    for (; i + 32 <= lcnt; i += 32) exact_step(i, 32);
+    if (lcnt >= 32) {
+      uint32_t q = W.list[lane];
+      float4 bb = fbox[q & 0xFFFFu];
+      for (; i + 32 <= lcnt; i += 32) {
+        uint32_t qn = 0;
+        float4 bn = bb;
+        if (i + 64 <= lcnt) { qn = W.list[i + 32 + lane]; bn = fbox[qn & 0xFFFFu]; }
+        if (kCount) ++n_exact;
+        const bool hit = iou_exceeds(W.rowbox[q >> 16], bb, cst);
+        if (kCount && hit) ++n_edge;
+        stage_hits(hit, q);
+        q = qn; bb = bn;
+      }
+    }
     const int rem = lcnt - i;
-    if (rem > 0 && all) { exact_step(i, rem); lcnt = 0; return; }
+    if (rem > 0 && all) {
+      bool hit = false;
+      uint32_t q = 0;
+      if (lane < rem) {
+        q = W.list[i + lane];
+        if (kCount) ++n_exact;
+        hit = iou_exceeds(W.rowbox[q >> 16], fbox[q & 0xFFFFu], cst);
+        if (kCount && hit) ++n_edge;
+      }
+      stage_hits(hit, q);
+      lcnt = 0;
+      return;
+    }
     if (rem > 0 && i > 0) {
       const uint32_t v = lane < rem ? W.list[i + lane] : 0u;
       __syncwarp();
