@@ -200,8 +200,8 @@ int schedule(ffpp_handle* h, int B, const int32_t* N, const int32_t* dims, cudaS
     fr[f] = d;
     coff[f] = cand;
     cand += n; cells += (int64_t)d.gw * d.gh;
-    d.k5_th = k5_tile_h(d.gw, d.gh);
-    d.k5_tiles = k5_tiles(d.gw, d.gh);
+    d.k5_th = k5_tile_h(d.gw, d.gh, h->cst.radius_t);
+    d.k5_tiles = k5_tiles(d.gw, d.gh, h->cst.radius_t);
     fr[f] = d;
     max_tiles = std::max(max_tiles, (int)d.k5_tiles);
     max_nmax = std::max(max_nmax, (int)d.nmax);

@@ -1200,56 +1200,62 @@ __global__ void __launch_bounds__(K4E_THREADS) k4e_emit(const FrameDesc* __restr
 // a6 — density convolution (north_star (d); the paper's grid-cell x bird loop,
 // PAPER.md:L203-208, restated as histogram + separable convolution).
 // One CTA per tile of th output rows x up to K5_TW output columns of one frame; th (a multiple of 16, chosen per grid
-// width by the host scheduler, FrameDesc::k5_th) makes a tile ~8 k cells whatever the grid width.  Everything after one
-// coalesced read of the uint16 histogram happens in shared memory:
+// width by the host scheduler, FrameDesc::k5_th) gives every thread exactly one y-pass unit.  Everything after one
+// coalesced read of the uint16 histogram happens in shared memory and registers, in 64 registers per thread so that
+// four CTAs share an SM and one tile's staging latency hides behind another tile's arithmetic:
 //  (1) stage: rows y0-RT .. y0+th+RT-1 of the histogram (reflect-folded at the top / bottom of the grid) are copied
-//      as they are, 16 bytes per cp.async (LDGSTS: asynchronous, no register staging);
+//      as they are, 16 bytes per cp.async (LDGSTS: asynchronous, no register staging); a thread owns one 8-column
+//      group and walks down the rows;
 //  (2) y pass: a thread owns TWO adjacent columns and 16 consecutive output rows: one 32-bit shared load brings a
-//      pair of counts, two byte-permutes + two subtractions turn them into floats (the 2^23 trick: full-rate ALU, no
-//      I2F), and the 16 pairs of sums are updated with packed fma.rn.f32x2 (FFMA2: two fp32 FMAs per issue slot; the
-//      (w_k, w_k) tap pairs stay in registers).  Columns outside the grid are not computed: the reflect border makes
-//      them copies of columns inside, filled in by a mirror pass, so the y pass does exactly (2R+1) FMAs per cell;
-//  (3) x pass: a thread reads 8 + 2 RT consecutive floats of one row (16-byte loads, row pitch = 4 mod 32 so a quarter
-//      warp of eight rows is conflict-free) and produces eight consecutive outputs; the taps are consumed two at a
-//      time, (w_k, w_k+1) x (v_j, v_j+1) on the aligned register pairs the loads deliver (the even / odd partial sums
-//      are added at the end), again FFMA2; one 32-byte sector is written per thread (two 16-byte stores when the
-//      address allows, whatever the caller's base pointer).
-// Radii above K5_PACKED_MAX_RT (tap pairs would not fit the register file) take scalar FMAs with constant-bank taps.
+//      pair of counts, two byte-permutes + one packed subtraction turn them into floats (the 2^23 trick: no I2F), and
+//      the 16 pairs of sums are updated with packed fma.rn.f32x2 (FFMA2: two fp32 FMAs per issue slot).  The kernel
+//      is symmetric, so only RT + 1 (w_k, w_k) tap pairs live in registers.  The sums stay in registers across a
+//      barrier and are then written OVER the staged histogram (the two arrays share their shared memory) as
+//      s_t[row pair][column] = (t[2p][x], t[2p+1][x]);
+//  (3) mirror: window columns outside the grid are reflections of computed ones (reflect border, O7);
+//  (4) x pass: a thread owns one ROW PAIR and eight consecutive columns: the packed lanes are now the two rows, so the
+//      same (w_k, w_k) tap pairs serve and an output costs exactly 2 RT + 1 FFMA2 per two cells; 16-byte shared loads
+//      (row-pair pitch = 2 mod 4 float2: a quarter warp of eight row pairs is conflict-free), two 32-byte sectors
+//      written per thread.
+// Radii above K5_PACKED_MAX_RT (the tap pairs would not fit the register file) take scalar FMAs with constant-bank taps.
 // The tap loops are fully unrolled for the compile-time radius bucket RT >= R (taps zero-padded to RT).
 // HBM traffic: 2 bytes per cell of histogram (L2 hits: a4 wrote it microseconds earlier) + one 4-byte store per cell.
 // =====================================================================================================
 constexpr int K5_THREADS = 256;
 constexpr int K5_TW = 256;                      // output columns per CTA at most (wider grids are tiled in x)
-constexpr int K5_PACKED_MAX_RT = 10;
+constexpr int K5_PACKED_MAX_RT = 12;
+constexpr int K5_RB = 16;                       // output rows of one y-pass unit
 
 __host__ __device__ inline int k5_tile_w(int gw) { return gw < K5_TW ? ((gw + 7) & ~7) : K5_TW; }      // multiple of 8
-__host__ __device__ inline int k5_tile_h(int gw, int gh) {                // multiple of 16: ~one y-pass unit per thread
-  const int npair = k5_tile_w(gw) / 2;
-  int nb = (K5_THREADS + npair / 2) / npair;
+// column pairs the y pass of one tile computes at most (an x-tiled grid adds the RT halo columns on both sides)
+__host__ __device__ inline int k5_npair_max(int gw, int RT) { return gw <= K5_TW ? (gw + 1) / 2 : (K5_TW + 2 * RT) / 2 + 1; }
+__host__ __device__ inline int k5_tile_h(int gw, int gh, int RT) {        // multiple of 16; units of the y pass <= K5_THREADS
+  int nb = K5_THREADS / k5_npair_max(gw, RT);
   if (nb < 1) nb = 1;
   const int cap = (gh + 15) & ~15;
-  return 16 * nb < cap ? 16 * nb : cap;
+  return K5_RB * nb < cap ? K5_RB * nb : cap;
 }
-__host__ __device__ inline int k5_pitch_t(int tw, int RT) {               // >= tw + 2 RT + 4, = 4 mod 32
-  const int need = tw + 2 * RT + 4;
-  return ((need - 4 + 31) / 32) * 32 + 4;
+__host__ __device__ inline int k5_pitch_t(int tw, int RT) {               // float2 per row pair: >= tw + 2 RT + 2, = 2 mod 4
+  const int need = tw + 2 * RT + 2;
+  return ((need - 2 + 3) / 4) * 4 + 2;
 }
 __host__ __device__ inline int k5_pitch_h(int tw, int RT) { return (tw + 2 * RT + 7 + 8 + 7) & ~7; }  // staged uint16 columns, multiple of 8
-__host__ __device__ inline size_t k5_tile_smem(int tw, int th, int RT) {
-  const size_t hb = (sizeof(uint16_t) * (size_t)(th + 2 * RT) * k5_pitch_h(tw, RT) + 15) & ~(size_t)15;
-  return hb + sizeof(float) * (size_t)th * k5_pitch_t(tw, RT);
+__host__ __device__ inline size_t k5_tile_smem(int tw, int th, int RT) {  // the two arrays alias
+  const size_t hb = sizeof(uint16_t) * (size_t)(th + 2 * RT) * k5_pitch_h(tw, RT);
+  const size_t tb = sizeof(float2) * (size_t)(th / 2) * k5_pitch_t(tw, RT);
+  return ((hb > tb ? hb : tb) + 15) & ~(size_t)15;
 }
 __host__ __device__ inline size_t k5_smem_bytes(int gw_max, int gh_max, int RT) {   // largest tile any grid up to gw_max x gh_max needs
   size_t m = 0;
   for (int gw = 8; gw <= ((gw_max + 7) & ~7); gw += 8) {
-    const size_t b = k5_tile_smem(k5_tile_w(gw), k5_tile_h(gw, gh_max), RT);
+    const size_t b = k5_tile_smem(k5_tile_w(gw), k5_tile_h(gw, gh_max, RT), RT);
     if (b > m) m = b;
   }
   return m;
 }
 __host__ __device__ inline int k5_tiles_x(int gw) { const int tw = k5_tile_w(gw); return (gw + tw - 1) / tw; }
-__host__ __device__ inline int k5_tiles(int gw, int gh) {
-  const int th = k5_tile_h(gw, gh);
+__host__ __device__ inline int k5_tiles(int gw, int gh, int RT) {
+  const int th = k5_tile_h(gw, gh, RT);
   return k5_tiles_x(gw) * ((gh + th - 1) / th);
 }
 
@@ -1261,10 +1267,10 @@ __device__ __forceinline__ void cp_async16(void* dst_smem, const void* src_gmem)
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst_smem)), "l"(src_gmem) : "memory");
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
-// u / d for 0 <= u < 2^20 with inv = 1.0f / d: (u + 0.5) / d is at least 0.5 / d away from every integer, far more than
+// u / d for 0 <= u < 2^20 with inv = the correctly rounded 1 / d: (u + 0.5) / d is at least 0.5 / d away from every integer, far more than
 // the rounding error of the product
 __device__ __forceinline__ int fast_div(const int u, const float inv) { return (int)(((float)u + 0.5f) * inv); }
-// packed fp32 pairs (FFMA2)
+// packed fp32 pairs (FFMA2 / FADD2)
 __device__ __forceinline__ unsigned long long pk2(const float lo, const float hi) {
   unsigned long long r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r;
 }
@@ -1272,13 +1278,17 @@ __device__ __forceinline__ void unpk2(const unsigned long long v, float& lo, flo
 __device__ __forceinline__ unsigned long long fma2(const unsigned long long a, const unsigned long long b, const unsigned long long c) {
   unsigned long long d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d;
 }
+__device__ __forceinline__ unsigned long long add2(const unsigned long long a, const unsigned long long b) {
+  unsigned long long d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d;
+}
 
 template <int RT>
-__global__ void __launch_bounds__(K5_THREADS) k5_density(const FrameDesc* __restrict__ frames, Consts cst,
-                                                         const uint16_t* __restrict__ hist16,
-                                                         float* __restrict__ out_density) {
+__global__ void __launch_bounds__(K5_THREADS, (RT <= K5_PACKED_MAX_RT ? 4 : 2)) k5_density(const FrameDesc* __restrict__ frames, Consts cst,
+                                                                                         const uint16_t* __restrict__ hist16,
+                                                                                         float* __restrict__ out_density) {
   extern __shared__ __align__(16) uint8_t s_k5[];
   constexpr bool kPacked = RT <= K5_PACKED_MAX_RT;
+  constexpr int RB = K5_RB, NW = RB + 2 * RT;
   const int f = blockIdx.y;
   const FrameDesc* fd = &frames[f];
   if ((int)blockIdx.x >= fd->k5_tiles) return;
@@ -1292,103 +1302,107 @@ __global__ void __launch_bounds__(K5_THREADS) k5_density(const FrameDesc* __rest
   const int sx0 = cx0 & ~7;                                  // first staged column (16-byte copies)
   const int Ph = k5_pitch_h(tw, RT), Pt = k5_pitch_t(tw, RT);
   uint16_t* s_h = reinterpret_cast<uint16_t*>(s_k5);         // [th + 2 RT][Ph]: staged histogram rows, column gx - sx0
-  float* s_t = reinterpret_cast<float*>(s_k5 + ((sizeof(uint16_t) * (size_t)(th + 2 * RT) * Ph + 15) & ~(size_t)15));
-  constexpr int OD = RT & 1;                                 // s_t[y][ct]: ct = gx - (x0 - RT) + OD, so even gx <-> even ct
+  unsigned long long* s_t = reinterpret_cast<unsigned long long*>(s_k5);   // [th / 2][Pt] (t[2p][x], t[2p+1][x]); ALIASES s_h
+  constexpr int OD = RT & 1;                                 // s_t column of grid column gx: gx - (x0 - RT) + OD (even gx <-> even column)
   const int tid = threadIdx.x;
   const uint16_t* hsrc = hist16 + fd->dens_off;
 
-  // ---- (1) stage: 8 cells (16 bytes) per copy ----
+  // ---- (1) stage: 8 cells (16 bytes) per copy; a thread keeps its column group and walks down the rows ----
   {
-    const int ng = (cx1 - sx0 + 7) >> 3;                    // 8-column groups per row
+    const int ng = (cx1 - sx0 + 7) >> 3;                    // 8-column groups per row (<= 37)
     const int nrows = th + 2 * RT;
-    const float inv = 1.0f / (float)ng;
+    const float inv_ng = __frcp_rn((float)ng);
+    const int rstep = fast_div(K5_THREADS, inv_ng);
+    const int r0 = fast_div(tid, inv_ng), g = tid - r0 * ng;
     const bool vec = (((uintptr_t)hsrc & 15) == 0) && ((gw & 7) == 0);
-    for (int u = tid; u < ng * nrows; u += K5_THREADS) {
-      const int r = fast_div(u, inv), g = u - r * ng;
-      const int gy = k5_fold(y0 - RT + r, gh);
+    if (r0 < rstep) {
       const int gx = sx0 + 8 * g;
-      const uint16_t* src = hsrc + gy * gw + gx;
-      uint16_t* dst = s_h + r * Ph + 8 * g;
-      if (vec) {                                            // gw % 8 == 0: a group never straddles the row end
-        cp_async16(dst, src);
+      uint16_t* dst = s_h + r0 * Ph + 8 * g;
+      if (vec && y0 - RT >= 0 && y0 + th + RT <= gh) {        // interior tile: no fold, one pointer bump per copy
+        const uint16_t* src = hsrc + (y0 - RT + r0) * gw + gx;
+        uint32_t d32 = smem_u32(dst);
+        for (int r = r0; r < nrows; r += rstep, d32 += (uint32_t)(rstep * Ph * 2), src += rstep * gw)
+          asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d32), "l"(src) : "memory");
       } else {
+        for (int r = r0; r < nrows; r += rstep, dst += rstep * Ph) {
+          const uint16_t* src = hsrc + k5_fold(y0 - RT + r, gh) * gw + gx;
+          if (vec) {                                          // gw % 8 == 0: a group never straddles the row end
+            cp_async16(dst, src);
+          } else {
 #pragma unroll
-        for (int e = 0; e < 8; ++e) dst[e] = gx + e < gw ? src[e] : (uint16_t)0;
+            for (int e = 0; e < 8; ++e) dst[e] = gx + e < gw ? src[e] : (uint16_t)0;
+          }
+        }
       }
     }
     cp_async_wait_all();
   }
   __syncthreads();
 
-  // ---- (2) y pass ----
-  {
-    const int px0 = cx0 & ~1;                               // pairs start on an even column (>= sx0)
-    const int npair = (cx1 - px0 + 1) >> 1;
-    const float inv = 1.0f / (float)npair;
-    if constexpr (kPacked) {
-      constexpr int RB = 16, NW = RB + 2 * RT;
-      unsigned long long wp[2 * RT + 1];
+  // ---- (2) y pass: one unit (column pair, 16 rows) per thread, sums in registers ----
+  const int px0 = cx0 & ~1;                                 // pairs start on an even column (>= sx0)
+  const int npair = (cx1 - px0 + 1) >> 1;
+  const int q = fast_div(tid, __frcp_rn((float)npair)), c = tid - q * npair;
+  const bool yact = q < th / RB && y0 + RB * q < gh;       // else: no such unit, or a block of rows below the grid
+  unsigned long long wp[kPacked ? RT + 1 : 1];              // (w_k, w_k) for k = 0 .. RT; w_(2RT - k) = w_k
+  if constexpr (kPacked) {
 #pragma unroll
-      for (int k = 0; k <= 2 * RT; ++k) wp[k] = pk2(cst.taps_pad[k], cst.taps_pad[k]);
-      for (int u = tid; u < npair * (th / RB); u += K5_THREADS) {
-        const int q = fast_div(u, inv), c = u - q * npair;
-        if (y0 + RB * q >= gh) continue;                    // a block of rows below the grid (last tile of a frame)
-        const uint32_t* col = reinterpret_cast<const uint32_t*>(s_h + (RB * q) * Ph + (px0 - sx0) + 2 * c);
-        unsigned long long acc[RB];
+    for (int k = 0; k <= RT; ++k) wp[k] = pk2(cst.taps_pad[k], cst.taps_pad[k]);
+  }
+  unsigned long long acc[RB];
 #pragma unroll
-        for (int m = 0; m < RB; ++m) acc[m] = 0ull;
+  for (int m = 0; m < RB; ++m) acc[m] = 0ull;
+  if (yact) {
+    const uint32_t* col = reinterpret_cast<const uint32_t*>(s_h + (RB * q) * Ph + (px0 - sx0) + 2 * c);
+    const unsigned long long magic = pk2(-8388608.0f, -8388608.0f);
 #pragma unroll
-        for (int r = 0; r < NW; ++r) {
-          const uint32_t v = col[r * (Ph / 2)];
-          // count -> float without I2F: 0x4B000000 | c is the float 2^23 + c
-          const float v0 = __uint_as_float(__byte_perm(v, 0x4B000000u, 0x7610)) - 8388608.0f;
-          const float v1 = __uint_as_float(__byte_perm(v, 0x4B000000u, 0x7632)) - 8388608.0f;
-          const unsigned long long vv = pk2(v0, v1);
+    for (int r = 0; r < NW; ++r) {
+      const uint32_t v = col[r * (Ph / 2)];
+      // count -> float without I2F: 0x4B000000 | c is the float 2^23 + c
+      unsigned long long vv = pk2(__uint_as_float(__byte_perm(v, 0x4B000000u, 0x7610)), __uint_as_float(__byte_perm(v, 0x4B000000u, 0x7632)));
+      if constexpr (kPacked) {
+        vv = add2(vv, magic);
 #pragma unroll
-          for (int m = 0; m < RB; ++m) {
-            const int k = r - m;                            // compile-time after unrolling
-            if (k >= 0 && k <= 2 * RT) acc[m] = fma2(wp[k], vv, acc[m]);
+        for (int m = 0; m < RB; ++m) {
+          const int k = r - m;                              // compile-time after unrolling
+          if (k >= 0 && k <= 2 * RT) acc[m] = fma2(wp[k <= RT ? k : 2 * RT - k], vv, acc[m]);
+        }
+      } else {
+        float v0, v1;
+        unpk2(vv, v0, v1);
+        v0 -= 8388608.0f; v1 -= 8388608.0f;
+#pragma unroll
+        for (int m = 0; m < RB; ++m) {
+          const int k = r - m;
+          if (k >= 0 && k <= 2 * RT) {
+            float a0, a1;
+            unpk2(acc[m], a0, a1);
+            acc[m] = pk2(fmaf(cst.taps_pad[k], v0, a0), fmaf(cst.taps_pad[k], v1, a1));
           }
         }
-        unsigned long long* dst = reinterpret_cast<unsigned long long*>(s_t + (RB * q) * Pt + (px0 - (x0 - RT) + OD) + 2 * c);
-#pragma unroll
-        for (int m = 0; m < RB; ++m) dst[m * (Pt / 2)] = acc[m];
-      }
-    } else {
-      constexpr int RB = 8, NW = RB + 2 * RT;
-      for (int u = tid; u < npair * (th / RB); u += K5_THREADS) {
-        const int q = fast_div(u, inv), c = u - q * npair;
-        if (y0 + RB * q >= gh) continue;
-        const uint32_t* col = reinterpret_cast<const uint32_t*>(s_h + (RB * q) * Ph + (px0 - sx0) + 2 * c);
-        float a0[RB], a1[RB];
-#pragma unroll
-        for (int m = 0; m < RB; ++m) { a0[m] = 0.0f; a1[m] = 0.0f; }
-#pragma unroll
-        for (int r = 0; r < NW; ++r) {
-          const uint32_t v = col[r * (Ph / 2)];
-          const float v0 = __uint_as_float(__byte_perm(v, 0x4B000000u, 0x7610)) - 8388608.0f;
-          const float v1 = __uint_as_float(__byte_perm(v, 0x4B000000u, 0x7632)) - 8388608.0f;
-#pragma unroll
-          for (int m = 0; m < RB; ++m) {
-            const int k = r - m;
-            if (k >= 0 && k <= 2 * RT) { a0[m] = fmaf(cst.taps_pad[k], v0, a0[m]); a1[m] = fmaf(cst.taps_pad[k], v1, a1[m]); }
-          }
-        }
-        float2* dst = reinterpret_cast<float2*>(s_t + (RB * q) * Pt + (px0 - (x0 - RT) + OD) + 2 * c);
-#pragma unroll
-        for (int m = 0; m < RB; ++m) dst[m * (Pt / 2)] = make_float2(a0[m], a1[m]);
       }
     }
   }
+  __syncthreads();                                          // every read of the staged histogram is done: s_t may overwrite it
+  if (yact) {
+    // acc[m] = (t[m][2c], t[m][2c+1]) -> rows paired: (t[m][2c], t[m+1][2c]), (t[m][2c+1], t[m+1][2c+1]): one 16-byte store
+    ulonglong2* dst = reinterpret_cast<ulonglong2*>(s_t + (RB / 2 * q) * Pt + (px0 - (x0 - RT) + OD) + 2 * c);
+#pragma unroll
+    for (int m = 0; m < RB; m += 2) {
+      float a0, a1, b0, b1;
+      unpk2(acc[m], a0, a1); unpk2(acc[m + 1], b0, b1);
+      dst[(m / 2) * (Pt / 2)] = make_ulonglong2(pk2(a0, b0), pk2(a1, b1));
+    }
+  }
   __syncthreads();
-  // mirror pass: the columns of the window that lie outside the grid are reflections of computed ones
+  // ---- (3) mirror pass: the columns of the window that lie outside the grid are reflections of computed ones ----
   {
     const int nct = (x1 - x0) + 2 * RT;
     const int lo = cx0 - (x0 - RT), hi = cx1 - (x0 - RT);   // computed range, in window columns
     const int nfill = lo + (nct - hi);
     if (nfill) {                                            // block-uniform
-      const float inv = 1.0f / (float)nfill;
-      for (int u = tid; u < nfill * th; u += K5_THREADS) {
+      const float inv = __frcp_rn((float)nfill);
+      for (int u = tid; u < nfill * (th / 2); u += K5_THREADS) {
         const int y = fast_div(u, inv), e = u - y * nfill;
         const int wc = e < lo ? e : hi + (e - lo);
         const int gx = min(max(k5_fold(x0 - RT + wc, gw), cx0), cx1 - 1);
@@ -1398,72 +1412,62 @@ __global__ void __launch_bounds__(K5_THREADS) k5_density(const FrameDesc* __rest
     }
   }
 
-  // ---- (3) x pass: unit = (row y, 8-column group g); consecutive lanes take consecutive rows ----
+  // ---- (4) x pass: unit = (row pair p, 8-column group g); consecutive lanes take consecutive groups of one row pair,
+  // so a warp's stores cover whole 128-byte lines (the 4-way bank conflict of its 16-byte shared loads costs a few
+  // hundred cycles per tile; stores that scatter over 32 rows cost thousands) ----
   float* out = out_density + fd->dens_off;
   constexpr int NWX = 8 + 2 * RT;                           // window of one 8-output block
-  constexpr int NL = (NWX + OD + 3) / 4;
-  const float inv_th = 1.0f / (float)th;
-  unsigned long long wE[kPacked ? RT : 1], wO[kPacked ? RT : 1];
-  if constexpr (kPacked) {
-#pragma unroll
-    for (int j = 0; j < RT; ++j) {
-      wE[j] = pk2(cst.taps_pad[2 * j], cst.taps_pad[2 * j + 1]);
-      wO[j] = pk2(cst.taps_pad[2 * j + 1], cst.taps_pad[2 * j + 2]);
-    }
-  }
-  for (int u = tid; u < th * (tw / 8); u += K5_THREADS) {
-    const int g = fast_div(u, inv_th), y = u - g * th;
-    const int gy = y0 + y, gx = x0 + 8 * g;
+  constexpr int NL = (NWX + OD + 1) / 2;                    // 16-byte loads (two columns each)
+  const int ngrp = tw / 8;
+  const float inv_ngrp = __frcp_rn((float)ngrp);
+  for (int u = tid; u < (th / 2) * ngrp; u += K5_THREADS) {
+    const int yp = fast_div(u, inv_ngrp), g = u - yp * ngrp;
+    const int gy = y0 + 2 * yp, gx = x0 + 8 * g;
     if (gy >= gh || gx >= gw) continue;
-    float acc[8];
-    if constexpr (kPacked) {
-      const ulonglong2* row2 = reinterpret_cast<const ulonglong2*>(s_t + y * Pt + 8 * g);
-      unsigned long long P[2 * NL];                         // P[i] = (v[2i], v[2i+1])
+    const ulonglong2* row2 = reinterpret_cast<const ulonglong2*>(s_t + yp * Pt + 8 * g);
+    unsigned long long xa[8];
 #pragma unroll
-      for (int i = 0; i < NL; ++i) { const ulonglong2 t = row2[i]; P[2 * i] = t.x; P[2 * i + 1] = t.y; }
+    for (int m = 0; m < 8; ++m) xa[m] = 0ull;
 #pragma unroll
-      for (int m = 0; m < 8; ++m) {
-        constexpr int dummy = 0; (void)dummy;
-        const int s0 = OD + m;                              // window index of tap 0 (compile-time after unrolling)
-        unsigned long long a = 0ull;
-        float lo, hi, single;
-        if ((s0 & 1) == 0) {                                // taps (0,1), (2,3), ... on aligned pairs; tap 2 RT alone
+    for (int i = 0; i < NL; ++i) {
+      const ulonglong2 t2 = row2[i];
 #pragma unroll
-          for (int j = 0; j < RT; ++j) a = fma2(wE[j], P[s0 / 2 + j], a);
-          unpk2(P[s0 / 2 + RT], lo, hi);
-          single = cst.taps_pad[2 * RT] * lo;
-        } else {                                            // tap 0 alone; taps (1,2), (3,4), ... on aligned pairs
+      for (int h = 0; h < 2; ++h) {
+        const int r = 2 * i + h - OD;                       // window index (compile-time)
+        const unsigned long long vv = h ? t2.y : t2.x;
+        if (r >= 0 && r < NWX) {
 #pragma unroll
-          for (int j = 0; j < RT; ++j) a = fma2(wO[j], P[(s0 + 1) / 2 + j], a);
-          unpk2(P[(s0 - 1) / 2], lo, hi);
-          single = cst.taps_pad[0] * hi;
+          for (int m = 0; m < 8; ++m) {
+            const int k = r - m;
+            if (k >= 0 && k <= 2 * RT) {
+              if constexpr (kPacked) {
+                xa[m] = fma2(wp[k <= RT ? k : 2 * RT - k], vv, xa[m]);
+              } else {
+                float v0, v1, a0, a1;
+                unpk2(vv, v0, v1); unpk2(xa[m], a0, a1);
+                xa[m] = pk2(fmaf(cst.taps_pad[k], v0, a0), fmaf(cst.taps_pad[k], v1, a1));
+              }
+            }
+          }
         }
-        unpk2(a, lo, hi);
-        acc[m] = (lo + hi) + single;
-      }
-    } else {
-      const float4* row4 = reinterpret_cast<const float4*>(s_t + y * Pt + 8 * g);
-      float win[4 * NL];
-#pragma unroll
-      for (int i = 0; i < NL; ++i) {
-        const float4 t = row4[i];
-        win[4 * i] = t.x; win[4 * i + 1] = t.y; win[4 * i + 2] = t.z; win[4 * i + 3] = t.w;
-      }
-#pragma unroll
-      for (int m = 0; m < 8; ++m) {
-        acc[m] = 0.0f;
-#pragma unroll
-        for (int k = 0; k <= 2 * RT; ++k) acc[m] = fmaf(cst.taps_pad[k], win[OD + m + k], acc[m]);
       }
     }
-    float* dst = out + gy * gw + gx;
-    if ((((uintptr_t)dst & 15) == 0) && gx + 8 <= gw) {
-      reinterpret_cast<float4*>(dst)[0] = make_float4(acc[0], acc[1], acc[2], acc[3]);
-      reinterpret_cast<float4*>(dst)[1] = make_float4(acc[4], acc[5], acc[6], acc[7]);
-    } else {
+    float r0v[8], r1v[8];
 #pragma unroll
-      for (int m = 0; m < 8; ++m)
-        if (gx + m < gw) dst[m] = acc[m];
+    for (int m = 0; m < 8; ++m) unpk2(xa[m], r0v[m], r1v[m]);
+#pragma unroll
+    for (int rr = 0; rr < 2; ++rr) {
+      if (gy + rr >= gh) break;
+      const float* v = rr ? r1v : r0v;
+      float* dst = out + (gy + rr) * gw + gx;
+      if ((((uintptr_t)dst & 15) == 0) && gx + 8 <= gw) {
+        reinterpret_cast<float4*>(dst)[0] = make_float4(v[0], v[1], v[2], v[3]);
+        reinterpret_cast<float4*>(dst)[1] = make_float4(v[4], v[5], v[6], v[7]);
+      } else {
+#pragma unroll
+        for (int m = 0; m < 8; ++m)
+          if (gx + m < gw) dst[m] = v[m];
+      }
     }
   }
 }
