@@ -176,3 +176,52 @@ def make_config(c: int, seed_offset: int = 0, B: int | None = None, threads: int
     specs, kw = config_specs(c, B)
     return generate(f"config{c}" + (f"_B{B}" if B else ""), specs, seed=config_seed(c) + seed_offset, threads=threads,
                     iou_margin=iou_margin, **kw)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# Inputs of the SURVEY §8(f) rows f3 / f4 (numpy only; stand-ins for the paper's UNeXt segmentation output and its
+# 1080p / 720p farm video frames, PAPER.md:L70-76, L256, L278).  No method arithmetic: a probability mask is a sum of
+# seeded blobs, an image is seeded smooth colour noise.
+# ---------------------------------------------------------------------------------------------------------------
+def make_mask_batch(B: int, W: int, H: int, *, birds: float = 300.0, seed: int = 0x2512_0700_9, dtype="fp16") -> np.ndarray:
+    """[B, H, W] bird-segmentation probabilities in [0, 1]: Poisson(birds) elliptical blobs per frame (axes lognormal
+    around 14 x 9 px, random orientation, peak 0.6-0.99, soft edge), some touching, plus low-level background noise."""
+    rng = np.random.default_rng(seed)
+    out = np.empty((B, H, W), dtype=np.float16 if dtype == "fp16" else np.float32)
+    yy, xx = np.mgrid[0:H, 0:W].astype(np.float32)
+    for b in range(B):
+        m = rng.random((H, W), dtype=np.float32) * 0.25                 # background: well below any sane threshold ...
+        speck = rng.random((H, W)) < 2e-4                               # ... plus isolated hot pixels (1-pixel components)
+        m[speck] = 0.9
+        nb = int(rng.poisson(birds))
+        cx = rng.uniform(0, W, nb); cy = rng.uniform(0, H, nb)
+        a = 14.0 * np.exp(rng.normal(0, 0.25, nb)); bb = 9.0 * np.exp(rng.normal(0, 0.25, nb))
+        th = rng.uniform(0, np.pi, nb); pk = rng.uniform(0.6, 0.99, nb)
+        for i in range(nb):
+            x0, x1 = int(max(0, cx[i] - 3 * a[i])), int(min(W, cx[i] + 3 * a[i] + 1))
+            y0, y1 = int(max(0, cy[i] - 3 * a[i])), int(min(H, cy[i] + 3 * a[i] + 1))
+            if x0 >= x1 or y0 >= y1:
+                continue
+            dx = xx[y0:y1, x0:x1] - cx[i]; dy = yy[y0:y1, x0:x1] - cy[i]
+            u = (dx * np.cos(th[i]) + dy * np.sin(th[i])) / a[i]
+            v = (-dx * np.sin(th[i]) + dy * np.cos(th[i])) / bb[i]
+            blob = pk[i] / (1.0 + np.exp(8.0 * (np.sqrt(u * u + v * v) - 1.0)))      # soft-edged ellipse
+            np.maximum(m[y0:y1, x0:x1], blob.astype(np.float32), out=m[y0:y1, x0:x1])
+        out[b] = m
+    return out
+
+
+def make_image_batch(B: int, W: int, H: int, *, seed: int = 0x2512_0700_9) -> np.ndarray:
+    """[B, H, W, 3] uint8 frames: smooth colour gradients + blocks + pixel noise (every byte value occurs)."""
+    rng = np.random.default_rng(seed)
+    yy, xx = np.mgrid[0:H, 0:W].astype(np.float32)
+    out = np.empty((B, H, W, 3), dtype=np.uint8)
+    for b in range(B):
+        for c in range(3):
+            fx, fy, ph = rng.uniform(0.002, 0.05), rng.uniform(0.002, 0.05), rng.uniform(0, 6.28)
+            img = 127.5 + 100.0 * np.sin(fx * xx + fy * yy + ph) + rng.normal(0, 12.0, (H, W))
+            out[b, :, :, c] = np.clip(img, 0, 255).astype(np.uint8)
+        for _ in range(8):                                              # hard-edged blocks (sharp transitions)
+            x0, y0 = int(rng.integers(0, W)), int(rng.integers(0, H))
+            out[b, y0:y0 + int(rng.integers(4, 64)), x0:x0 + int(rng.integers(4, 64)), :] = rng.integers(0, 256, 3, dtype=np.uint8)
+    return out

@@ -1,4 +1,4 @@
-"""ctypes binding of the CPU oracle (oracle/ffpp_oracle.cpp) — TEST INFRASTRUCTURE.
+"""ctypes binding of the CPU oracle (oracle/ffpp_oracle.cpp, oracle/ffpp_next_oracle.cpp) — TEST INFRASTRUCTURE.
 
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs import
 this.  It imports nothing from the CUDA package and the CUDA package imports nothing from here.
@@ -15,6 +15,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "ffpp_oracle.cpp")
 _LIB = os.path.join(_HERE, "libffpp_oracle.so")
+_SRC_NEXT = os.path.join(_HERE, "ffpp_next_oracle.cpp")
+_LIB_NEXT = os.path.join(_HERE, "libffpp_next_oracle.so")
 
 
 class OracleParams(ctypes.Structure):
@@ -33,6 +35,9 @@ def build(force: bool = False) -> str:
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         subprocess.check_call(["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-fno-fast-math", "-fPIC", "-shared",
                                "-o", _LIB, _SRC])
+    if force or not os.path.exists(_LIB_NEXT) or os.path.getmtime(_LIB_NEXT) < os.path.getmtime(_SRC_NEXT):
+        subprocess.check_call(["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-fno-fast-math", "-fPIC", "-shared",
+                               "-o", _LIB_NEXT, _SRC_NEXT])
     return _LIB
 
 
@@ -166,3 +171,84 @@ def run(params: dict, raw: np.ndarray, N_per_frame, frame_dims) -> Result:
     if rc != 0:
         raise RuntimeError(f"oracle_run failed: {rc}")
     return r
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# SURVEY §8(f) f1-f4 (oracle/ffpp_next_oracle.cpp)
+# ---------------------------------------------------------------------------------------------------------------
+REGION_DTYPE = np.dtype([("label", "<i4"), ("area", "<i4"), ("x0", "<i4"), ("y0", "<i4"), ("x1", "<i4"), ("y1", "<i4"),
+                         ("mass", "<f4"), ("reserved_", "<i4")])
+
+_lib_next = None
+
+
+def lib_next():
+    global _lib_next
+    if _lib_next is None:
+        build()
+        L = ctypes.CDLL(_LIB_NEXT)
+        vp, i32, i64, f32 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_float
+        L.oracle_entropy.restype = ctypes.c_double
+        L.oracle_entropy.argtypes = [vp, i64]
+        L.oracle_clustering_degree.restype = ctypes.c_double
+        L.oracle_clustering_degree.argtypes = [vp, i64]
+        L.oracle_regions.restype = i32
+        L.oracle_regions.argtypes = [vp, i32, i32, f32, i32, vp, vp, i32]
+        L.oracle_density_exact.restype = i32
+        L.oracle_density_exact.argtypes = [vp, i32, i32, i32, i32, f32, f32, vp]
+        L.oracle_mask_components.restype = i32
+        L.oracle_mask_components.argtypes = [vp, i32, i32, i32, f32, i32, i32, vp, vp, i32]
+        L.oracle_preprocess.restype = None
+        L.oracle_preprocess.argtypes = [vp, i32, i32, i32, i32, vp, vp, vp]
+        _lib_next = L
+    return _lib_next
+
+
+def entropy(D) -> float:
+    d = np.ascontiguousarray(D, dtype=np.float32).reshape(-1)
+    return float(lib_next().oracle_entropy(_ptr(d), d.size))
+
+
+def clustering_degree(D) -> float:
+    d = np.ascontiguousarray(D, dtype=np.float32).reshape(-1)
+    return float(lib_next().oracle_clustering_degree(_ptr(d), d.size))
+
+
+def regions(D, thr: float, conn: int = 4, max_regions: int = 4096):
+    """(labels [gh, gw] int32, table REGION_DTYPE[min(count, max_regions)], count)."""
+    d = np.ascontiguousarray(D, dtype=np.float32)
+    gh, gw = d.shape
+    labels = np.zeros((gh, gw), dtype=np.int32)
+    tab = np.zeros(max_regions, dtype=REGION_DTYPE)
+    n = lib_next().oracle_regions(_ptr(d), gw, gh, thr, conn, _ptr(labels), _ptr(tab), max_regions)
+    return labels, tab[:min(n, max_regions)].copy(), int(n)
+
+
+def density_exact(boxes, W: int, H: int, cell: int, sigma: float, truncate: float = 3.0):
+    b = np.ascontiguousarray(boxes, dtype=np.float32).reshape(-1, 4)
+    out = np.zeros((H // cell, W // cell), dtype=np.float32)
+    n_in = lib_next().oracle_density_exact(_ptr(b), len(b), W, H, cell, sigma, truncate, _ptr(out))
+    return out, int(n_in)
+
+
+def mask_components(mask, thr: float, conn: int = 8, min_area: int = 1, max_components: int = 8192):
+    """mask [H, W] float16/float32 -> (labels [H, W] int32, table REGION_DTYPE (mass = mean probability), count)."""
+    m = np.ascontiguousarray(mask)
+    assert m.dtype in (np.float16, np.float32) and m.ndim == 2
+    H, W = m.shape
+    labels = np.zeros((H, W), dtype=np.int32)
+    tab = np.zeros(max_components, dtype=REGION_DTYPE)
+    n = lib_next().oracle_mask_components(_ptr(m), 1 if m.dtype == np.float16 else 0, W, H, thr, conn, min_area, _ptr(labels),
+                                          _ptr(tab), max_components)
+    return labels, tab[:min(n, max_components)].copy(), int(n)
+
+
+def preprocess(img, Hd: int, Wd: int, mean, std) -> np.ndarray:
+    """img [Hs, Ws, 3] uint8 -> [3, Hd, Wd] float64."""
+    a = np.ascontiguousarray(img, dtype=np.uint8)
+    Hs, Ws, _ = a.shape
+    mean = np.ascontiguousarray(mean, dtype=np.float32)
+    std = np.ascontiguousarray(std, dtype=np.float32)
+    out = np.zeros((3, Hd, Wd), dtype=np.float64)
+    lib_next().oracle_preprocess(_ptr(a), Hs, Ws, Hd, Wd, _ptr(mean), _ptr(std), _ptr(out))
+    return out
