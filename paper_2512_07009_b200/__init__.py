@@ -22,7 +22,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 _LIB = os.path.join(_HERE, "libffpp.so")
-_SOURCES = ["ffpp.cu", "ffpp_kernels.cuh", "ffpp_common.cuh"]
+_SOURCES = ["ffpp.cu", "ffpp_kernels.cuh", "ffpp_common.cuh", "ffpp_next.cuh"]
 _INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
@@ -49,6 +49,10 @@ BOX_DTYPE = np.dtype([("x1", "<f4"), ("y1", "<f4"), ("x2", "<f4"), ("y2", "<f4")
 EXPORTS = ["ffpp_create", "ffpp_run", "ffpp_run_host", "ffpp_destroy", "ffpp_last_error", "ffpp_get_info",
            "ffpp_set_stage_timing", "ffpp_get_stage_ms"]
 DEBUG_EXPORTS = ["ffpp_debug_read", "ffpp_debug_count_work", "ffpp_debug_stream_read"]     # include/ffpp_debug.h
+NEXT_EXPORTS = ["ffpp_heatmap_stats", "ffpp_density_exact", "ffpp_mask_components", "ffpp_preprocess"]   # include/ffpp_next.h
+
+REGION_DTYPE = np.dtype([("label", "<i4"), ("area", "<i4"), ("x0", "<i4"), ("y0", "<i4"), ("x1", "<i4"), ("y1", "<i4"),
+                         ("mass", "<f4"), ("reserved_", "<i4")])
 
 
 class FFPPParams(ctypes.Structure):
@@ -78,7 +82,7 @@ class FFPPError(RuntimeError):
 
 def build(force: bool = False, verbose: bool = False) -> str:
     """Compile csrc/ffpp.cu for sm_100a into libffpp.so next to this file (nvcc cross-compiles without a GPU)."""
-    srcs = [os.path.join(_CSRC, s) for s in _SOURCES] + [os.path.join(_INCLUDE, "ffpp.h"), os.path.join(_INCLUDE, "ffpp_debug.h")]
+    srcs = [os.path.join(_CSRC, s) for s in _SOURCES] + [os.path.join(_INCLUDE, "ffpp.h"), os.path.join(_INCLUDE, "ffpp_debug.h"), os.path.join(_INCLUDE, "ffpp_next.h")]
     stale = not os.path.exists(_LIB) or any(os.path.getmtime(s) > os.path.getmtime(_LIB) for s in srcs)
     if force or stale:
         cmd = ["nvcc"] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", _LIB, os.path.join(_CSRC, "ffpp.cu")]
@@ -118,6 +122,15 @@ def load_library() -> ctypes.CDLL:
         L.ffpp_debug_count_work.argtypes = [vp, i32]
         L.ffpp_debug_stream_read.restype = ctypes.c_int
         L.ffpp_debug_stream_read.argtypes = [vp, vp, i64, vp]
+        f32 = ctypes.c_float
+        L.ffpp_heatmap_stats.restype = ctypes.c_int
+        L.ffpp_heatmap_stats.argtypes = [vp, vp, i32, vp, f32, i32, i32, vp, vp, vp, vp, vp, vp]
+        L.ffpp_density_exact.restype = ctypes.c_int
+        L.ffpp_density_exact.argtypes = [vp, vp, vp, i32, vp, vp, vp]
+        L.ffpp_mask_components.restype = ctypes.c_int
+        L.ffpp_mask_components.argtypes = [vp, vp, i32, i32, i32, i32, f32, i32, i32, i32, vp, vp, vp, vp]
+        L.ffpp_preprocess.restype = ctypes.c_int
+        L.ffpp_preprocess.argtypes = [vp, i32, i32, i32, i32, i32, vp, vp, i32, vp, vp]
         _lib = L
     return _lib
 
@@ -306,3 +319,72 @@ class FFPP:
             a = np.zeros((B, K, 4), dtype=np.float32)
         self._check(self._lib.ffpp_debug_read(self._h, what, a.ctypes.data, a.nbytes))
         return a
+
+
+    # ---- SURVEY §8(f) f1-f3 (include/ffpp_next.h): argument marshalling only ----
+    def heatmap_stats(self, density, frame_dims, threshold: float, *, connectivity: int = 4, max_regions: int = 1024, stream=None):
+        """ffpp_heatmap_stats.  density: CUDA float32 tensor in ffpp_run's out_density layout.  Returns a dict of CUDA
+        tensors: entropy [B] f64, degree [B] f64, labels [cells] i32, regions [B, max_regions, 8] i32 (view with
+        REGION_DTYPE), region_counts [B] i32."""
+        torch = self._torch
+        dims = self._host_i32(frame_dims, (-1, 2))
+        B = int(dims.shape[0])
+        assert density.is_cuda and density.dtype == torch.float32 and density.is_contiguous()
+        res = {"entropy": torch.empty(B, dtype=torch.float64, device="cuda"), "degree": torch.empty(B, dtype=torch.float64, device="cuda"),
+               "labels": torch.empty(density.numel(), dtype=torch.int32, device="cuda"),
+               "regions": torch.zeros((B, max_regions, 8), dtype=torch.int32, device="cuda"),
+               "region_counts": torch.empty(B, dtype=torch.int32, device="cuda")}
+        st = stream if stream is not None else torch.cuda.current_stream()
+        self._check(self._lib.ffpp_heatmap_stats(self._h, density.data_ptr(), B, dims.ctypes.data, threshold, connectivity, max_regions,
+                                                 st.cuda_stream, res["entropy"].data_ptr(), res["degree"].data_ptr(), res["labels"].data_ptr(),
+                                                 res["regions"].data_ptr(), res["region_counts"].data_ptr()))
+        return res
+
+    def density_exact(self, out: Output, frame_dims, stream=None):
+        """ffpp_density_exact on the kept boxes of a finished run; returns a CUDA float32 tensor in the out_density layout."""
+        torch = self._torch
+        dims = self._host_i32(frame_dims, (-1, 2))
+        B = int(dims.shape[0])
+        dens = torch.empty(int(self.density_offsets(dims)[-1]), dtype=torch.float32, device="cuda")
+        st = stream if stream is not None else torch.cuda.current_stream()
+        self._check(self._lib.ffpp_density_exact(self._h, out.boxes.data_ptr(), out.counts.data_ptr(), B, dims.ctypes.data, st.cuda_stream,
+                                                 dens.data_ptr()))
+        return dens
+
+    def mask_components(self, mask, threshold: float, *, connectivity: int = 8, min_area: int = 1, max_components: int = 4096, stream=None):
+        """ffpp_mask_components.  mask: CUDA tensor [B, H, W] float16/float32.  Returns dict: labels [B, H, W] i32,
+        components [B, max_components, 8] i32 (REGION_DTYPE; mass = mean probability), counts [B] i32."""
+        torch = self._torch
+        assert mask.is_cuda and mask.is_contiguous() and mask.dim() == 3 and mask.dtype in (torch.float16, torch.float32)
+        B, H, W = (int(v) for v in mask.shape)
+        res = {"labels": torch.empty((B, H, W), dtype=torch.int32, device="cuda"),
+               "components": torch.zeros((B, max_components, 8), dtype=torch.int32, device="cuda"),
+               "counts": torch.empty(B, dtype=torch.int32, device="cuda")}
+        st = stream if stream is not None else torch.cuda.current_stream()
+        self._check(self._lib.ffpp_mask_components(self._h, mask.data_ptr(), 1 if mask.dtype == torch.float16 else 0, B, W, H, threshold,
+                                                   connectivity, min_area, max_components, st.cuda_stream, res["labels"].data_ptr(),
+                                                   res["components"].data_ptr(), res["counts"].data_ptr()))
+        return res
+
+
+def regions_numpy(t) -> np.ndarray:
+    """[B, max, 8] int32 CUDA/CPU tensor of ffpp_region records -> numpy structured array [B, max]."""
+    a = t.cpu().numpy() if hasattr(t, "cpu") else np.asarray(t)
+    return np.ascontiguousarray(a).view(REGION_DTYPE).reshape(a.shape[0], a.shape[1])
+
+
+def preprocess(src, Hd: int, Wd: int, mean, std, *, out_dtype="fp16", stream=None):
+    """ffpp_preprocess.  src: CUDA uint8 tensor [B, Hs, Ws, 3] -> CUDA tensor [B, 3, Hd, Wd] float16/float32."""
+    import torch
+    lib = load_library()
+    assert src.is_cuda and src.dtype == torch.uint8 and src.is_contiguous() and src.dim() == 4 and src.shape[3] == 3
+    B, Hs, Ws, _ = (int(v) for v in src.shape)
+    dst = torch.empty((B, 3, Hd, Wd), dtype=torch.float16 if out_dtype == "fp16" else torch.float32, device="cuda")
+    m = np.ascontiguousarray(mean, dtype=np.float32)
+    s = np.ascontiguousarray(std, dtype=np.float32)
+    st = stream if stream is not None else torch.cuda.current_stream()
+    rc = lib.ffpp_preprocess(src.data_ptr(), B, Hs, Ws, Hd, Wd, m.ctypes.data, s.ctypes.data, 1 if out_dtype == "fp16" else 0, st.cuda_stream,
+                             dst.data_ptr())
+    if rc != FFPP_OK:
+        raise FFPPError(rc, "ffpp_preprocess")
+    return dst

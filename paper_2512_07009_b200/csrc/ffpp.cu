@@ -93,6 +93,23 @@ struct ffpp_handle {
   cudaStream_t s_h2d = nullptr, s_d2h = nullptr;     // copy streams of the chunked host path (created on first use)
   static constexpr int kHostChunks = 8;
   cudaEvent_t ev_up[kHostChunks] = {}, ev_run[kHostChunks] = {};
+  // SURVEY §8(f) f1-f3 (ffpp_next.cuh): cached grid tables of f1 / f2 and the component-labelling scratch (grown on demand)
+  struct NextGeo {
+    void* d_tab = nullptr;
+    uint64_t hash = 0, last_use = 0;
+    int B = -1;
+    std::vector<int32_t> dims;
+    int64_t cells = 0;
+    int max_cells = 0, max_w = 0, max_h = 0;
+  };
+  static constexpr int kNextSlots = 8;
+  NextGeo ngeo[kNextSlots];
+  int32_t* d_ccl_aux = nullptr;
+  int64_t ccl_aux_cap = 0;
+  unsigned long long* d_ccl_sums = nullptr;
+  int64_t ccl_sum_cap = 0;
+  void* d_ent_part = nullptr;
+  int64_t ent_part_cap = 0;
   // stage timing
   bool timing = false;
   cudaEvent_t ev[FFPP_NUM_STAGES + 1] = {};
@@ -630,6 +647,8 @@ int ffpp_destroy(ffpp_handle* h) {
   cudaFree(h->d_sp_key); cudaFree(h->d_cellstart); cudaFree(h->d_hasin); cudaFree(h->d_k4_scratch); cudaFree(h->d_kept_key); cudaFree(h->d_kept_pos); cudaFree(h->d_edges);
   cudaFree(h->d_hist32);
   cudaFree(h->d_in); cudaFree(h->d_out_boxes); cudaFree(h->d_out_counts); cudaFree(h->d_out_density);
+  for (int sl = 0; sl < ffpp_handle::kNextSlots; ++sl) cudaFree(h->ngeo[sl].d_tab);
+  cudaFree(h->d_ccl_aux); cudaFree(h->d_ccl_sums); cudaFree(h->d_ent_part);
   if (h->s_h2d) cudaStreamDestroy(h->s_h2d);
   if (h->s_d2h) cudaStreamDestroy(h->s_d2h);
   for (int i = 0; i < ffpp_handle::kHostChunks; ++i) { if (h->ev_up[i]) cudaEventDestroy(h->ev_up[i]); if (h->ev_run[i]) cudaEventDestroy(h->ev_run[i]); }
@@ -759,3 +778,5 @@ int ffpp_debug_phases(unsigned long long* dst, int frames) {
 #endif
 
 }  // extern "C"
+
+#include "ffpp_next.cuh"

@@ -22,7 +22,9 @@ def test_library_builds_loads_and_exports_the_header():
     dbg = declared_symbols("ffpp_debug.h")
     assert set(dbg) == set(m.DEBUG_EXPORTS), (dbg, m.DEBUG_EXPORTS)
     assert not [s for s in syms if "debug" in s], "include/ffpp.h is the contract only"
-    for s in syms + dbg:
+    nxt = declared_symbols("ffpp_next.h")
+    assert set(nxt) == set(m.NEXT_EXPORTS), (nxt, m.NEXT_EXPORTS)
+    for s in syms + dbg + nxt:
         assert hasattr(lib, s), f"libffpp.so does not export {s}"
     # null-handle calls that need no device
     lib.ffpp_destroy.argtypes = [ctypes.c_void_p]
