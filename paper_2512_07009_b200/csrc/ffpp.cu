@@ -108,6 +108,8 @@ struct ffpp_handle {
   int64_t ccl_aux_cap = 0;
   unsigned long long* d_ccl_sums = nullptr;
   int64_t ccl_sum_cap = 0;
+  int32_t* d_ccl_blk = nullptr;
+  int64_t ccl_blk_cap = 0;
   void* d_ent_part = nullptr;
   int64_t ent_part_cap = 0;
   // stage timing
@@ -648,7 +650,7 @@ int ffpp_destroy(ffpp_handle* h) {
   cudaFree(h->d_hist32);
   cudaFree(h->d_in); cudaFree(h->d_out_boxes); cudaFree(h->d_out_counts); cudaFree(h->d_out_density);
   for (int sl = 0; sl < ffpp_handle::kNextSlots; ++sl) cudaFree(h->ngeo[sl].d_tab);
-  cudaFree(h->d_ccl_aux); cudaFree(h->d_ccl_sums); cudaFree(h->d_ent_part);
+  cudaFree(h->d_ccl_aux); cudaFree(h->d_ccl_sums); cudaFree(h->d_ccl_blk); cudaFree(h->d_ent_part);
   if (h->s_h2d) cudaStreamDestroy(h->s_h2d);
   if (h->s_d2h) cudaStreamDestroy(h->s_d2h);
   for (int i = 0; i < ffpp_handle::kHostChunks; ++i) { if (h->ev_up[i]) cudaEventDestroy(h->ev_up[i]); if (h->ev_run[i]) cudaEventDestroy(h->ev_run[i]); }

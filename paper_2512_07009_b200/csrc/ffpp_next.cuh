@@ -32,8 +32,8 @@ __device__ __forceinline__ float load_prob(const __half* p, const int64_t i) { r
 //   kc_init    label = own index / -1, area counter = 0
 //   kc_merge   unions
 //   kc_flatten label = root; area[root] += 1
-//   kc_rank    one CTA per image: ordered compaction of the roots with area >= min_area into the table (ascending
-//              label), the table index of every root goes to the counter array
+//   kr_*       ordered compaction of the roots with area >= min_area into the table (ascending label); the table
+//              index of every root goes to the counter array
 //   kc_stats   bounding box (atomicMin / atomicMax) and sum (64-bit fixed point, 2^-40: order-independent, so
 //              bit-reproducible) of every listed component; a warp whose pixels all belong to one component
 //              reduces first and issues one set of atomics
@@ -50,9 +50,20 @@ __global__ void __launch_bounds__(KC_THREADS) kc_init(const T* __restrict__ src,
   const ImgDesc d = img_desc(tab, blockIdx.y, w0, h0);
   const int n = d.w * d.h;
   const int i = blockIdx.x * KC_THREADS + threadIdx.x;
-  if (i >= n) return;
-  labels[d.off + i] = load_prob(src, d.off + i) > thr ? i : -1;
-  aux[d.off + i] = 0;
+  if (blockIdx.x * KC_THREADS >= n) return;
+  const int lane = threadIdx.x & 31;
+  const bool valid = i < n;
+  const bool fg = valid && load_prob(src, d.off + i) > thr;
+  // horizontal runs inside the warp's 32 consecutive pixels start labelled with the run's first pixel: the unions
+  // along a row are done before the first atomic (a run that continues from the previous warp is united in kc_merge)
+  const int x = valid ? i % d.w : 0;
+  const uint32_t bits = __ballot_sync(0xffffffffu, fg), rowstart = __ballot_sync(0xffffffffu, valid && x == 0);
+  const uint32_t starts = bits & (~(bits << 1) | rowstart);
+  const int first = 31 - __clz((int)(starts & (0xFFFFFFFFu >> (31 - lane))));
+  if (valid) {
+    labels[d.off + i] = fg ? i - (lane - first) : -1;
+    aux[d.off + i] = 0;
+  }
 }
 
 __device__ __forceinline__ int cc_find(const int32_t* L, int i) {
@@ -74,20 +85,34 @@ __device__ __forceinline__ void cc_unite(int32_t* L, int a, int b) {
   }
 }
 
+// Unions between rows, one per START of a vertical contact instead of one per pixel: with the left neighbour and the
+// upper-left neighbour both foreground, the left neighbour (or a pixel further left in the same run) has already
+// joined the two rows.  Under 8-connectivity a diagonal contact counts only where the pixel straight above is
+// background (otherwise the upper run already holds both), and only from the end of the run that touches it.
 __global__ void __launch_bounds__(KC_THREADS) kc_merge(const ImgDesc* __restrict__ tab, int w0, int h0, int conn, int32_t* __restrict__ labels) {
   const ImgDesc d = img_desc(tab, blockIdx.y, w0, h0);
   const int w = d.w, n = d.w * d.h;
   const int i = blockIdx.x * KC_THREADS + threadIdx.x;
-  if (i >= n) return;
+  if (blockIdx.x * KC_THREADS >= n) return;
+  const int lane = threadIdx.x & 31;
   int32_t* L = labels + d.off;
-  if (L[i] < 0) return;
+  const bool valid = i < n;
+  const bool fg = valid && L[i] >= 0;                        // foreground never changes: label >= 0
+  const uint32_t bits = __ballot_sync(0xffffffffu, fg);
+  if (!fg) return;
   const int y = i / w, x = i - y * w;
-  if (x > 0 && L[i - 1] >= 0) cc_unite(L, i, i - 1);
-  if (y > 0) {
-    if (L[i - w] >= 0) cc_unite(L, i, i - w);
-    if (conn == 8) {
-      if (x > 0 && L[i - w - 1] >= 0) cc_unite(L, i, i - w - 1);
-      if (x + 1 < w && L[i - w + 1] >= 0) cc_unite(L, i, i - w + 1);
+  const bool left = x > 0 && (lane > 0 ? ((bits >> (lane - 1)) & 1u) != 0 : L[i - 1] >= 0);
+  if (lane == 0 && left) cc_unite(L, i, i - 1);              // the run continues from the previous warp
+  if (y == 0) return;
+  const bool up = L[i - w] >= 0;
+  const bool ul = x > 0 && L[i - w - 1] >= 0;
+  if (up) {
+    if (!(left && ul)) cc_unite(L, i, i - w);
+  } else if (conn == 8) {
+    if (ul && !left) cc_unite(L, i, i - w - 1);
+    if (x + 1 < w && L[i - w + 1] >= 0) {
+      const bool right = lane < 31 ? ((bits >> (lane + 1)) & 1u) != 0 : (i + 1 < n && L[i + 1] >= 0);
+      if (!right) cc_unite(L, i, i - w + 1);
     }
   }
 }
@@ -107,66 +132,101 @@ __global__ void __launch_bounds__(KC_THREADS) kc_flatten(const ImgDesc* __restri
   if ((int)(__ffs(peers) - 1) == (int)(threadIdx.x & 31)) atomicAdd(&aux[d.off + r], __popc(peers));
 }
 
-// entropy partial sums ride along with the ranking CTA's inputs: see ke_partial below
-__global__ void __launch_bounds__(KC_RANK_THREADS) kc_rank(const ImgDesc* __restrict__ tab, int w0, int h0, const int32_t* __restrict__ labels,
-                                                           int32_t* __restrict__ aux, int min_area, int max_out,
-                                                           ffpp_region* __restrict__ out, unsigned long long* __restrict__ sums,
-                                                           int32_t* __restrict__ out_counts) {
-  __shared__ int s_wsum[2][KC_RANK_THREADS / 32];
-  const int img = blockIdx.x;
+// Ordered compaction of the roots with area >= min_area into the table (ascending label), in three launches so that a
+// 2 M-pixel mask is scanned by hundreds of CTAs: per block of 4096 pixels the number of listed roots (kr_count), per
+// image the exclusive scan of the block counts (kr_scan), per block the table rows (kr_place).  The table index of every
+// root replaces its area in the counter array (-1: not listed).
+constexpr int KR_BLOCK = KC_RANK_THREADS * KC_RANK_PER;
+
+__device__ __forceinline__ int kr_block_scan(const int c, int* s_wsum, const int tid, int* total) {   // exclusive prefix of c over the CTA
+  const int lane = tid & 31, warp = tid >> 5;
+  int inc = c;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
+  if (lane == 31) s_wsum[warp] = inc;
+  __syncthreads();
+  const int wv = s_wsum[lane];
+  int winc = wv;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, winc, o); if (lane >= o) winc += t; }
+  *total = __shfl_sync(0xffffffffu, winc, 31);
+  return __shfl_sync(0xffffffffu, winc - wv, warp) + inc - c;
+}
+
+template <bool kPlace>
+__global__ void __launch_bounds__(KC_RANK_THREADS) kr_count_place(const ImgDesc* __restrict__ tab, int w0, int h0, const int32_t* __restrict__ labels,
+                                                                  int32_t* __restrict__ aux, int min_area, int max_out, int nblk_max,
+                                                                  int32_t* __restrict__ blk, ffpp_region* __restrict__ out,
+                                                                  unsigned long long* __restrict__ sums) {
+  __shared__ int s_wsum[KC_RANK_THREADS / 32];
+  const int img = blockIdx.y;
   const ImgDesc d = img_desc(tab, img, w0, h0);
   const int n = d.w * d.h;
+  const int base = blockIdx.x * KR_BLOCK;
+  if (base >= n) return;
   const int32_t* L = labels + d.off;
   int32_t* A = aux + d.off;
+  const int tid = threadIdx.x;
+  const int i0 = base + tid * KC_RANK_PER;
+  int area[KC_RANK_PER];
+  uint32_t rootm = 0, selm = 0;
+#pragma unroll
+  for (int e = 0; e < KC_RANK_PER; ++e) {
+    const int i = i0 + e;
+    area[e] = 0;
+    if (i < n && L[i] == i) {
+      rootm |= 1u << e;
+      area[e] = A[i];
+      if (area[e] >= min_area) selm |= 1u << e;
+    }
+  }
+  int total;
+  const int excl = kr_block_scan(__popc(selm), s_wsum, tid, &total);
+  if (!kPlace) {
+    if (tid == 0) blk[(int64_t)img * nblk_max + blockIdx.x] = total;
+    return;
+  }
   ffpp_region* table = out + (int64_t)img * max_out;
   unsigned long long* sm = sums + (int64_t)img * max_out;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  int running = 0, par = 0;
-  for (int base = 0; base < n; base += KC_RANK_THREADS * KC_RANK_PER, par ^= 1) {
-    const int i0 = base + tid * KC_RANK_PER;
-    int area[KC_RANK_PER];
-    uint32_t rootm = 0, selm = 0;
+  int pos = blk[(int64_t)img * nblk_max + blockIdx.x] + excl;
 #pragma unroll
-    for (int e = 0; e < KC_RANK_PER; ++e) {
-      const int i = i0 + e;
-      area[e] = 0;
-      if (i < n && L[i] == i) {
-        rootm |= 1u << e;
-        area[e] = A[i];
-        if (area[e] >= min_area) selm |= 1u << e;
+  for (int e = 0; e < KC_RANK_PER; ++e) {
+    if (!((rootm >> e) & 1u)) continue;
+    const int i = i0 + e;
+    int k = -1;
+    if ((selm >> e) & 1u) {
+      if (pos < max_out) {
+        k = pos;
+        ffpp_region r;
+        r.label = i; r.area = area[e]; r.x0 = INT_MAX; r.y0 = INT_MAX; r.x1 = -1; r.y1 = -1; r.mass = 0.0f; r.reserved_ = 0;
+        table[k] = r;
+        sm[k] = 0ull;
       }
+      ++pos;
     }
-    const int c = __popc(selm);
-    int inc = c;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
-    if (lane == 31) s_wsum[par][warp] = inc;
-    __syncthreads();
-    const int wv = s_wsum[par][lane];
-    int winc = wv;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, winc, o); if (lane >= o) winc += t; }
-    const int before = __shfl_sync(0xffffffffu, winc - wv, warp);
-    const int total = __shfl_sync(0xffffffffu, winc, 31);
-    int pos = running + before + inc - c;
-#pragma unroll
-    for (int e = 0; e < KC_RANK_PER; ++e) {
-      if (!((rootm >> e) & 1u)) continue;
-      const int i = i0 + e;
-      int k = -1;
-      if ((selm >> e) & 1u) {
-        if (pos < max_out) {
-          k = pos;
-          ffpp_region r;
-          r.label = i; r.area = area[e]; r.x0 = INT_MAX; r.y0 = INT_MAX; r.x1 = -1; r.y1 = -1; r.mass = 0.0f; r.reserved_ = 0;
-          table[k] = r;
-          sm[k] = 0ull;
-        }
-        ++pos;
-      }
-      A[i] = k;                                              // table index of this root, -1 if not listed
-    }
+    A[i] = k;                                                // table index of this root, -1 if not listed
+  }
+}
+
+__global__ void __launch_bounds__(KC_THREADS) kr_scan(const ImgDesc* __restrict__ tab, int w0, int h0, int nblk_max, int32_t* __restrict__ blk,
+                                                      int32_t* __restrict__ out_counts) {
+  __shared__ int s_wsum[32];
+  const int img = blockIdx.x;
+  const ImgDesc d = img_desc(tab, img, w0, h0);
+  const int nblk = (d.w * d.h + KR_BLOCK - 1) / KR_BLOCK;
+  int32_t* b = blk + (int64_t)img * nblk_max;
+  const int tid = threadIdx.x;
+  if (tid < 32) s_wsum[tid] = 0;                             // kr_block_scan reads 32 warp sums; this CTA has 8 warps
+  __syncthreads();
+  int running = 0;
+  for (int base = 0; base < nblk; base += KC_THREADS) {
+    const int k = base + tid;
+    const int c = k < nblk ? b[k] : 0;
+    int total;
+    const int excl = kr_block_scan(c, s_wsum, tid, &total);
+    if (k < nblk) b[k] = running + excl;
     running += total;
+    __syncthreads();
   }
   if (tid == 0) out_counts[img] = running;
 }
@@ -468,8 +528,8 @@ int next_geometry(ffpp_handle* h, int B, const int32_t* dims, cudaStream_t st, c
 }
 
 // scratch of the component labelling: one int32 per pixel, one 64-bit sum per table row; grown on demand
-int next_scratch(ffpp_handle* h, int64_t pixels, int64_t rows, cudaStream_t st) {
-  if (pixels > h->ccl_aux_cap || rows > h->ccl_sum_cap) {
+int next_scratch(ffpp_handle* h, int64_t pixels, int64_t rows, int64_t blocks, cudaStream_t st) {
+  if (pixels > h->ccl_aux_cap || rows > h->ccl_sum_cap || blocks > h->ccl_blk_cap) {
     cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
     if (cudaStreamIsCapturing(st, &cap) == cudaSuccess && cap != cudaStreamCaptureStatusNone)
       return fail(h, FFPP_EINVAL, "labelling scratch not allocated yet: run this call once outside stream capture first");
@@ -487,6 +547,12 @@ int next_scratch(ffpp_handle* h, int64_t pixels, int64_t rows, cudaStream_t st) 
     FFPP_CUDA(h, cudaMalloc((void**)&h->d_ccl_sums, sizeof(unsigned long long) * (size_t)rows));
     h->ccl_sum_cap = rows;
   }
+  if (blocks > h->ccl_blk_cap) {
+    FFPP_CUDA(h, cudaStreamSynchronize(st));
+    cudaFree(h->d_ccl_blk); h->d_ccl_blk = nullptr; h->ccl_blk_cap = 0;
+    FFPP_CUDA(h, cudaMalloc((void**)&h->d_ccl_blk, sizeof(int32_t) * (size_t)blocks));
+    h->ccl_blk_cap = blocks;
+  }
   return FFPP_OK;
 }
 
@@ -498,7 +564,11 @@ int run_ccl(ffpp_handle* h, const T* src, const ffpp::ImgDesc* tab, int B, int w
   kc_init<T><<<g, KC_THREADS, 0, st>>>(src, tab, w0, h0, thr, labels, h->d_ccl_aux);
   kc_merge<<<g, KC_THREADS, 0, st>>>(tab, w0, h0, conn, labels);
   kc_flatten<<<g, KC_THREADS, 0, st>>>(tab, w0, h0, labels, h->d_ccl_aux);
-  kc_rank<<<B, KC_RANK_THREADS, 0, st>>>(tab, w0, h0, labels, h->d_ccl_aux, min_area, max_out, out, h->d_ccl_sums, counts);
+  const int nblk = (max_px + KR_BLOCK - 1) / KR_BLOCK;
+  const dim3 gr((unsigned)nblk, (unsigned)B);
+  kr_count_place<false><<<gr, KC_RANK_THREADS, 0, st>>>(tab, w0, h0, labels, h->d_ccl_aux, min_area, max_out, nblk, h->d_ccl_blk, out, h->d_ccl_sums);
+  kr_scan<<<B, KC_THREADS, 0, st>>>(tab, w0, h0, nblk, h->d_ccl_blk, counts);
+  kr_count_place<true><<<gr, KC_RANK_THREADS, 0, st>>>(tab, w0, h0, labels, h->d_ccl_aux, min_area, max_out, nblk, h->d_ccl_blk, out, h->d_ccl_sums);
   kc_stats<T><<<g, KC_THREADS, 0, st>>>(src, tab, w0, h0, labels, h->d_ccl_aux, max_out, out, h->d_ccl_sums);
   const dim3 gf((unsigned)((max_out + KC_THREADS - 1) / KC_THREADS), (unsigned)B);
   kc_final<<<gf, KC_THREADS, 0, st>>>(max_out, mean, counts, out, h->d_ccl_sums);
@@ -539,7 +609,7 @@ int ffpp_heatmap_stats(ffpp_handle* h, const float* density, int32_t B, const in
     FFPP_CUDA(h, cudaMalloc((void**)&h->d_ent_part, sizeof(double2) * (size_t)B * nblk));
     h->ent_part_cap = (int64_t)B * nblk;
   }
-  if ((rc = next_scratch(h, cells, (int64_t)B * max_regions, st)) != FFPP_OK) return rc;
+  if ((rc = next_scratch(h, cells, (int64_t)B * max_regions, (int64_t)B * ((max_cells + KR_BLOCK - 1) / KR_BLOCK), st)) != FFPP_OK) return rc;
   ke_partial<<<dim3((unsigned)nblk, (unsigned)B), KE_THREADS, 0, st>>>(density, tab, nblk, static_cast<double2*>(h->d_ent_part));
   ke_final<<<(B + 127) / 128, 128, 0, st>>>(tab, B, nblk, static_cast<const double2*>(h->d_ent_part), out_entropy, out_degree);
   return run_ccl<float>(h, density, tab, B, 0, 0, max_cells, threshold, connectivity, 1, max_regions, 0, st, out_labels, out_regions, out_region_counts);
@@ -584,7 +654,7 @@ int ffpp_mask_components(ffpp_handle* h, const void* mask, int32_t dtype, int32_
   if (max_components < 1) return fail(h, FFPP_EINVAL, "max_components must be >= 1");
   if (std::isnan(threshold)) return fail(h, FFPP_EINVAL, "threshold is NaN");
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  const int rc = next_scratch(h, (int64_t)B * W * H, (int64_t)B * max_components, st);
+  const int rc = next_scratch(h, (int64_t)B * W * H, (int64_t)B * max_components, (int64_t)B * ((W * H + KR_BLOCK - 1) / KR_BLOCK), st);
   if (rc != FFPP_OK) return rc;
   const int ma = min_area < 1 ? 1 : min_area;
   if (dtype == 1)
