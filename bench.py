@@ -49,10 +49,9 @@ CONFIG_DESC = {
     5: "config5: ragged B=256 (64 each 640x640/1280x1280/1920x1088/1280x720, interleaved) fp16, 6639360 candidates",
 }
 
-# fp32 lane-instructions of the a3 method's own work (DESIGN.md §6 a3): a culling-box test is four
-# compares, an exact IoU is 15 fp32 instructions (4 min/max, 2 sub, 2 clamp, 1 mul, 2 area mul, 2 area sub, add, sub,
+# fp32 lane-instructions of the a3 method's own work (DESIGN.md §6 a3): every candidate pair of the cell
+# windows gets the exact IoU, 15 fp32 instructions (4 min/max, 2 sub, 2 clamp, 1 mul, 2 area mul, 2 area sub, add, sub,
 # multiply-or-divide + compare)
-A3_OPS_PER_CULL_TEST = 4
 A3_OPS_PER_EXACT_IOU = 15
 FP32_LANES_PER_SM = 128
 
@@ -208,14 +207,14 @@ def reduce_over_ranks(total_ms: float, t_e2e: float, frames: float, cands: float
 
 def a3_roofline(work: np.ndarray, ms: float, sm_count: int, sm_mhz: float) -> dict:
     """Method's own fp32 lane-instructions of one a3 launch (device-counted) against the fp32 lane peak."""
-    ops = A3_OPS_PER_CULL_TEST * int(work[0]) + A3_OPS_PER_EXACT_IOU * int(work[1])
+    ops = A3_OPS_PER_EXACT_IOU * int(work[1])
     peak = sm_count * FP32_LANES_PER_SM * sm_mhz * 1e6
     ach = ops / (ms * 1e-3)
     return {"bound": "alu", "achieved": ach / 1e12, "peak": peak / 1e12, "unit": "T fp32 lane-instr/s", "frac": ach / peak,
-            "counted_work": {"culling_box_tests": int(work[0]), "exact_ious": int(work[1]), "edges": int(work[2]),
+            "counted_work": {"exact_ious": int(work[1]), "edges": int(work[2]),
                              "frames_on_overflow_path": int(work[3]), "lane_instructions": ops,
                              "how": "device counters of the counting instantiation of the a3 kernel, separate untimed run "
-                                    f"(ffpp_debug_count_work); {A3_OPS_PER_CULL_TEST} per culling test + {A3_OPS_PER_EXACT_IOU} per exact IoU"},
+                                    f"(ffpp_debug_count_work); {A3_OPS_PER_EXACT_IOU} per exact IoU"},
             "peak_source": f"{sm_count} SM x {FP32_LANES_PER_SM} fp32 lanes x {sm_mhz:.0f} MHz (sm_count from the handle, clocks.max.sm)"}
 
 
@@ -331,6 +330,115 @@ def quick_config(c: int, rank: int, flush, stream, hbm_peak: float) -> dict:
     return res
 
 
+
+# --------------------------------------------------------------------------------------------------------------
+# SURVEY §8(f) rows f1-f4 (include/ffpp_next.h): short cold-L2 measurements, reported beside the hot path
+# --------------------------------------------------------------------------------------------------------------
+def next_rows(b: "Bench", hbm_peak: float) -> dict:
+    import flockgen
+    torch, ffpp, pp, w, out = b.torch, b.ffpp, b.pp, b.w, b.out
+    stream = b.stream
+
+    def timed(fn, iters=8):
+        for _ in range(2):
+            fn()
+        torch.cuda.synchronize()
+        ts = []
+        for _ in range(iters):
+            b.flush_l2()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream); fn(); e1.record(stream)
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        return float(np.median(ts))
+
+    res = {}
+    b.step(); torch.cuda.synchronize()
+    cells = int(out.density_offsets[-1])
+    B = w.B
+    # f1: entropy, clustering degree, threshold + connected components on this batch's own density grids
+    MAXR = 512
+    h_ent = torch.empty(B, dtype=torch.float64, device="cuda"); h_deg = torch.empty(B, dtype=torch.float64, device="cuda")
+    h_lab = torch.empty(cells, dtype=torch.int32, device="cuda"); h_reg = torch.zeros((B, MAXR, 8), dtype=torch.int32, device="cuda")
+    h_cnt = torch.empty(B, dtype=torch.int32, device="cuda")
+    dims = np.ascontiguousarray(w.frame_dims, dtype=np.int32).reshape(-1, 2)
+
+    def f1():
+        rc = pp._lib.ffpp_heatmap_stats(pp._h, out.density.data_ptr(), B, dims.ctypes.data, 0.05, 4, MAXR, stream.cuda_stream,
+                                        h_ent.data_ptr(), h_deg.data_ptr(), h_lab.data_ptr(), h_reg.data_ptr(), h_cnt.data_ptr())
+        assert rc == 0, pp.last_error()
+    ms = timed(f1)
+    byt = 8 * cells + 32 * int(h_cnt.clamp(max=MAXR).sum())
+    res["f1_heatmap_stats"] = {"ms": ms, "workload": f"{B} density grids of this batch ({cells} cells), threshold 0.05, 4-connectivity",
+                               "regions": int(h_cnt.sum()), "mean_entropy_nats": float(h_ent.mean()), "mean_clustering_degree": float(h_deg.mean()),
+                               "algorithmic_bytes": byt, "GB/s": byt / (ms * 1e-3) / 1e9, "frac_of_hbm_peak": byt / (ms * 1e-3) / 1e9 / hbm_peak,
+                               "bytes_note": "4 B per cell read + 4 B per cell of label image written + 32 B per region",
+                               "kernels": "ke_partial ke_final kc_init kc_merge kc_flatten kr_count_place kr_scan kr_count_place kc_stats kc_final"}
+    # f2: exact-position density of the kept boxes, and what the binning of A14 costs against it
+    d_ex = torch.empty(cells, dtype=torch.float32, device="cuda")
+
+    def f2():
+        rc = pp._lib.ffpp_density_exact(pp._h, out.boxes.data_ptr(), out.counts.data_ptr(), B, dims.ctypes.data, stream.cuda_stream, d_ex.data_ptr())
+        assert rc == 0, pp.last_error()
+    ms = timed(f2)
+    diff = (d_ex - out.density).abs()
+    kept = int(out.counts.sum())
+    R = int(b.info.radius)
+    evals = kept * (2 * R + 1) ** 2
+    res["f2_density_exact"] = {"ms": ms, "workload": f"kept boxes of this batch ({kept}) onto {cells} cells", "cells_per_s": cells / (ms * 1e-3),
+                               "kernel_evaluations_needed": evals, "Gevals/s": evals / (ms * 1e-3) / 1e9,
+                               "binning_error_of_A14": {"max_abs": float(diff.max()), "mean_abs": float(diff.mean()),
+                                                        "max_density": float(d_ex.max()), "note": "|binned out_density - exact-position density| per cell (interior and border: the exact form has no fold)"},
+                               "kernels": "kd_exact"}
+    # f3: segmentation-mask post-processing, 8 masks of 1920x1080 fp16
+    MB, MW, MH, MAXC = 8, 1920, 1080, 4096
+    masks = torch.from_numpy(flockgen.make_mask_batch(MB, MW, MH, birds=800, seed=5)).cuda()
+    m_lab = torch.empty((MB, MH, MW), dtype=torch.int32, device="cuda"); m_tab = torch.zeros((MB, MAXC, 8), dtype=torch.int32, device="cuda")
+    m_cnt = torch.empty(MB, dtype=torch.int32, device="cuda")
+
+    def f3():
+        rc = pp._lib.ffpp_mask_components(pp._h, masks.data_ptr(), 1, MB, MW, MH, 0.5, 8, 20, MAXC, stream.cuda_stream, m_lab.data_ptr(),
+                                          m_tab.data_ptr(), m_cnt.data_ptr())
+        assert rc == 0, pp.last_error()
+    ms = timed(f3)
+    byt = 6 * MB * MW * MH
+    res["f3_mask_components"] = {"ms": ms, "ms_per_frame": ms / MB, "frames_per_s": MB / (ms * 1e-3),
+                                 "workload": f"{MB} synthetic 1920x1080 fp16 bird masks (~800 blobs each), threshold 0.5, 8-connectivity, min_area 20",
+                                 "components": int(m_cnt.sum()), "algorithmic_bytes": byt, "GB/s": byt / (ms * 1e-3) / 1e9,
+                                 "frac_of_hbm_peak": byt / (ms * 1e-3) / 1e9 / hbm_peak, "bytes_note": "2 B per pixel read + 4 B per pixel of label image written",
+                                 "paper_context": "paper: 40.2 -> 11.4 ms per frame on the CPU of a g4dn.2xlarge (PAPER.md:L151)",
+                                 "kernels": "kc_init kc_merge kc_flatten kr_count_place kr_scan kr_count_place kc_stats kc_final"}
+    del masks, m_lab
+    # f4: pre-processing, 8 frames of 1920x1080 -> 640x640 fp16 CHW, alone and overlapped with ffpp_run on a second stream
+    imgs = torch.from_numpy(flockgen.make_image_batch(MB, MW, MH, seed=5)).cuda()
+    dst = torch.empty((MB, 3, 640, 640), dtype=torch.float16, device="cuda")
+    mean = np.array([0.485, 0.456, 0.406], dtype=np.float32); std = np.array([0.229, 0.224, 0.225], dtype=np.float32)
+    lib = ffpp.load_library()
+
+    def f4(st=stream):
+        rc = lib.ffpp_preprocess(imgs.data_ptr(), MB, MH, MW, 640, 640, mean.ctypes.data, std.ctypes.data, 1, st.cuda_stream, dst.data_ptr())
+        assert rc == 0
+    ms = timed(f4)
+    byt = imgs.numel() + dst.numel() * 2
+    side = torch.cuda.Stream()
+
+    def serial():
+        f4(); b.step()
+
+    def overlapped():
+        side.wait_stream(stream)
+        f4(side)
+        b.step()
+        stream.wait_stream(side)
+    ms_serial, ms_overlap = timed(serial), timed(overlapped)
+    res["f4_preprocess"] = {"ms": ms, "ms_per_frame": ms / MB, "workload": f"{MB} frames 1920x1080x3 uint8 -> 640x640 fp16 CHW, ImageNet mean/std",
+                            "algorithmic_bytes": byt, "GB/s": byt / (ms * 1e-3) / 1e9, "frac_of_hbm_peak": byt / (ms * 1e-3) / 1e9 / hbm_peak,
+                            "bytes_note": "3 B per source pixel read once + 6 B per destination pixel written",
+                            "stream_overlap": {"ms_preprocess_then_ffpp_run_one_stream": ms_serial, "ms_preprocess_on_second_stream": ms_overlap,
+                                               "note": "next batch's pre-processing on a second stream while this batch's ffpp_run runs (PAPER.md:L308-310)"},
+                            "paper_context": "paper: 8.8 ms per frame (PAPER.md:L151)", "kernels": "kp_preprocess"}
+    return res
+
 # --------------------------------------------------------------------------------------------------------------
 # our arm
 # --------------------------------------------------------------------------------------------------------------
@@ -434,6 +542,14 @@ def run_ours(args):
                     configs[str(cc)] = quick_config(cc, rank, flush, stream, hbm_peak)
                 except Exception as exc:           # reported, never fatal for the main line
                     configs[str(cc)] = {"workload": CONFIG_DESC[cc], "error": str(exc)}
+
+    # ---- SURVEY §8(f) rows f1-f4 (single-GPU default run only) ----
+    nxt = {}
+    if world == 1 and not args.no_next:
+        try:
+            nxt = next_rows(b, hbm_peak)
+        except Exception as exc:                   # reported, never fatal for the main line
+            nxt = {"error": str(exc)}
 
     # ---- reduce over ranks ----
     total_ms, t_e2e, frames_all, cand_all = reduce_over_ranks(total_ms, t_e2e, float(B), float(total_cand), world, "cuda")
@@ -542,6 +658,7 @@ def run_ours(args):
             "cold_dirty_l2": {"ms_per_step": float(dirty_ms.sum()),
                               "note": "512 MB write only (round 1's regime): the first kernels compete with the write-back of dirty lines"},
             "configs": configs,
+            "next_rows": nxt,
             "cpu_baseline": cpu,
             "clocks": clocks,
             "workload_stats": {"survivors": int(n_surv.sum()), "entering_nms": int(n_sorted.sum()), "kept": kept_n,
@@ -562,6 +679,7 @@ def main():
     ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-other-configs", action="store_true", help="skip the short measurements of the other four configs")
+    ap.add_argument("--no-next", action="store_true", help="skip the measurements of the SURVEY 8(f) rows f1-f4")
     args = ap.parse_args()
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         return respawn_under_torchrun(args)
