@@ -91,7 +91,7 @@ struct ffpp_handle {
   int* d_out_counts = nullptr;
   float* d_out_density = nullptr;
   cudaStream_t s_h2d = nullptr, s_d2h = nullptr;     // copy streams of the chunked host path (created on first use)
-  static constexpr int kHostChunks = 8;
+  static constexpr int kHostChunks = 4;
   cudaEvent_t ev_up[kHostChunks] = {}, ev_run[kHostChunks] = {};
   // SURVEY §8(f) f1-f3 (ffpp_next.cuh): cached grid tables of f1 / f2 and the component-labelling scratch (grown on demand)
   struct NextGeo {
@@ -255,6 +255,20 @@ int schedule(ffpp_handle* h, int B, const int32_t* N, const int32_t* dims, cudaS
   return FFPP_OK;
 }
 
+// Launch `kern` as a programmatic dependent of the kernel before it in the stream: its launch is processed while the
+// predecessor still runs and it starts the moment the predecessor has finished (every such kernel begins with
+// pdl_wait()).  PAPER.md:L155: "many small and short-lived GPU kernels interspersed with idle gaps" — these are the gaps.
+template <typename... KArgs, typename... Args>
+cudaError_t launch_dep(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
+
 template <bool kHalf, typename KeyT>
 int launch_all(ffpp_handle* h, const void* raw, int B, cudaStream_t st, ffpp_box* out_boxes, int32_t* out_counts,
                float* out_density) {
@@ -277,39 +291,36 @@ int launch_all(ffpp_handle* h, const void* raw, int B, cudaStream_t st, ffpp_box
   }
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[2], st));
   // a2 (+ clears the a5 histogram)
-  k2_select_bin<kHalf, KeyT><<<B, K2_THREADS, k2_smem_bytes((size_t)c.top_k, sizeof(KeyT)), st>>>(
-      static_cast<const uint8_t*>(raw), frames, static_cast<const KeyT*>(h->d_surv_keys), h->surv_cnt(), c,
-      h->d_sel_box, h->d_sp_box, static_cast<KeyT*>(h->d_sp_key), h->d_cellstart, h->n_sorted(), h->d_hist32,
-      reinterpret_cast<uint32_t*>(h->d_hasin), h->sm_count);
+  launch_dep(k2_select_bin<kHalf, KeyT>, dim3((unsigned)B), dim3(K2_THREADS), k2_smem_bytes((size_t)c.top_k, sizeof(KeyT)), st,
+             static_cast<const uint8_t*>(raw), frames, static_cast<const KeyT*>(h->d_surv_keys), h->surv_cnt(), c,
+             h->d_sel_box, h->d_sp_box, static_cast<KeyT*>(h->d_sp_key), h->d_cellstart, h->n_sorted(), h->d_hist32,
+             reinterpret_cast<uint32_t*>(h->d_hasin), h->sm_count);
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[3], st));
   // a3 (+ the pool-free overflow path: its CTAs exit at once unless k3 flagged their frame)
   {
     const dim3 g3((unsigned)((g.max_nmax + K3_THREADS - 1) / K3_THREADS), (unsigned)B);
     if (g3.x > 0) {
       if (h->count_work)
-        k3_nms_edges<KeyT, true><<<g3, K3_THREADS, 0, st>>>(frames, h->n_sorted(), h->d_sp_box,
-                                                            static_cast<const KeyT*>(h->d_sp_key), h->d_cellstart, c,
-                                                            h->edge_ctr(), h->d_edges, h->d_hasin, h->frame_err(), h->d_work);
+        launch_dep(k3_nms_edges<KeyT, true>, g3, dim3(K3_THREADS), 0, st, frames, h->n_sorted(), h->d_sp_box,
+                   static_cast<const KeyT*>(h->d_sp_key), h->d_cellstart, c, h->edge_ctr(), h->d_edges, h->d_hasin, h->frame_err(), h->d_work);
       else
-        k3_nms_edges<KeyT, false><<<g3, K3_THREADS, 0, st>>>(frames, h->n_sorted(), h->d_sp_box,
-                                                             static_cast<const KeyT*>(h->d_sp_key), h->d_cellstart, c,
-                                                             h->edge_ctr(), h->d_edges, h->d_hasin, h->frame_err(), h->d_work);
-      k3o_overflow<KeyT><<<B, K3O_THREADS, (size_t)c.kpad, st>>>(frames, h->n_sorted(), h->d_sp_box,
-                                                                static_cast<const KeyT*>(h->d_sp_key), h->d_cellstart, c,
-                                                                h->edge_ctr(), h->d_hasin, h->frame_err());
+        launch_dep(k3_nms_edges<KeyT, false>, g3, dim3(K3_THREADS), 0, st, frames, h->n_sorted(), h->d_sp_box,
+                   static_cast<const KeyT*>(h->d_sp_key), h->d_cellstart, c, h->edge_ctr(), h->d_edges, h->d_hasin, h->frame_err(), h->d_work);
+      launch_dep(k3o_overflow<KeyT>, dim3((unsigned)B), dim3(K3O_THREADS), (size_t)c.kpad, st, frames, h->n_sorted(), h->d_sp_box,
+                 static_cast<const KeyT*>(h->d_sp_key), h->d_cellstart, c, h->edge_ctr(), h->d_hasin, h->frame_err());
     }
   }
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[4], st));
   // a4 (+ a5 histogram)
-  k4_resolve_order<KeyT><<<B, K4_THREADS, k4_smem_bytes((size_t)c.top_k, (size_t)c.kpad, sizeof(KeyT)), st>>>(
-      frames, h->n_sorted(), h->d_sp_box, static_cast<const KeyT*>(h->d_sp_key), h->edge_ctr(), h->d_edges,
-      reinterpret_cast<const uint32_t*>(h->d_hasin), c, h->sm_count, h->d_k4_scratch,
-      static_cast<KeyT*>(h->d_kept_key), h->d_kept_pos, out_counts);
+  launch_dep(k4_resolve_order<KeyT>, dim3((unsigned)B), dim3(K4_THREADS), k4_smem_bytes((size_t)c.top_k, (size_t)c.kpad, sizeof(KeyT)), st,
+             frames, h->n_sorted(), h->d_sp_box, static_cast<const KeyT*>(h->d_sp_key), h->edge_ctr(), h->d_edges,
+             reinterpret_cast<const uint32_t*>(h->d_hasin), c, h->sm_count, h->d_k4_scratch,
+             static_cast<KeyT*>(h->d_kept_key), h->d_kept_pos, out_counts);
   {
     const dim3 g4e((unsigned)((g.max_nmax + K4E_THREADS - 1) / K4E_THREADS), (unsigned)B);
     if (g4e.x > 0)
-      k4e_emit<KeyT><<<g4e, K4E_THREADS, 0, st>>>(frames, h->d_sp_box, static_cast<const KeyT*>(h->d_kept_key), h->d_kept_pos,
-                                                  out_counts, c, out_boxes, h->d_hist32);
+      launch_dep(k4e_emit<KeyT>, g4e, dim3(K4E_THREADS), 0, st, frames, h->d_sp_box, static_cast<const KeyT*>(h->d_kept_key), h->d_kept_pos,
+                 out_counts, c, out_boxes, h->d_hist32);
   }
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[5], st));
   // a6
@@ -318,7 +329,7 @@ int launch_all(ffpp_handle* h, const void* raw, int B, cudaStream_t st, ffpp_box
     const size_t s5 = k5_smem_bytes(h->p.max_frame_w / h->p.cell_px, h->p.max_frame_h / h->p.cell_px, c.radius_t);
     const uint16_t* h16 = reinterpret_cast<const uint16_t*>(h->d_hist32);
     switch (c.radius_t) {
-#define FFPP_K5_CASE(RT) case RT: k5_density<RT><<<g5, K5_THREADS, s5, st>>>(frames, c, h16, out_density); break;
+#define FFPP_K5_CASE(RT) case RT: launch_dep(k5_density<RT>, g5, dim3(K5_THREADS), s5, st, frames, c, h16, out_density); break;
       FFPP_K5_RADII(FFPP_K5_CASE)
 #undef FFPP_K5_CASE
       default: return fail(h, FFPP_EINVAL, "no a6 kernel for this radius");
@@ -558,10 +569,12 @@ int ffpp_run_host(ffpp_handle* h, const void* raw, int32_t B, const int32_t* N_p
   }
   // Frames are independent, so a large batch is cut BY BYTES into up to kHostChunks runs of whole frames: the upload of
   // run i+1 (copy stream) and the download of run i-1 (second copy stream) overlap the kernels of run i on `stream`.
-  // A run starts where the raw byte offset is a multiple of 16 (ffpp_run's alignment rule).  The last runs are the
-  // small ones: what is left after the final upload (its kernels + its download) is the un-overlapped tail.
+  // A run starts where the raw byte offset is a multiple of 16 (ffpp_run's alignment rule).  Four equal runs measured
+  // best on config 5 (1.61 ms against 2.06 with eight, 1.75 with three, 2.10 with one): a run's kernel chain costs
+  // 160-280 us however few frames it holds (one CTA per frame in a2 / a4), so more runs than four make the batch
+  // kernel-bound instead of PCIe-bound, and unequal shares only move that time around (profiles/r2_e2e_timeline.md).
   constexpr int kHostChunks = ffpp_handle::kHostChunks;
-  static const int kShare[kHostChunks] = {3, 3, 3, 3, 3, 2, 2, 1};            // of 20: relative raw bytes of the runs
+  static const int kShare[kHostChunks] = {5, 5, 5, 5};                        // of 20: relative raw bytes of the runs
   const size_t row = 5 * esz;
   std::vector<int> cut{0};                                          // first frame of every run, then B
   if (B >= 2 * kHostChunks && (size_t)cand * row >= ((size_t)16 << 20)) {

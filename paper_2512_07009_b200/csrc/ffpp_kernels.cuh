@@ -277,6 +277,7 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
     int* __restrict__ n_sorted, uint32_t* __restrict__ hist32, uint32_t* __restrict__ hasin, int sm_count) {
   constexpr int KB = sizeof(KeyT) * 8;
   extern __shared__ __align__(16) uint8_t smem[];
+  pdl_wait();
   const int K = cst.top_k;
   KeyT* sel = reinterpret_cast<KeyT*>(smem);
   uint32_t* aux = reinterpret_cast<uint32_t*>(sel + K);
@@ -552,6 +553,7 @@ __global__ void __launch_bounds__(K3_THREADS, 12) k3_nms_edges(const FrameDesc* 
   __shared__ K3Warp<KeyT> s_w[K3_WARPS];
   unsigned long long n_exact = 0, n_edge = 0;                 // kCount only: this lane's exact IoUs / edges
 
+  pdl_wait();
   const int f = blockIdx.y;
   const int n = n_sorted[f];
   const int p0 = blockIdx.x * K3_THREADS;
@@ -715,6 +717,7 @@ __global__ void __launch_bounds__(K3O_THREADS) k3o_overflow(const FrameDesc* __r
                                                             Consts cst, int* __restrict__ edge_ctr, uint8_t* __restrict__ hasin,
                                                             const int* __restrict__ frame_err) {
   extern __shared__ __align__(16) uint8_t s_state[];          // kpad bytes
+  pdl_wait();
   const int f = blockIdx.x;
   if (!frame_err[f]) return;
   const int n = n_sorted[f];
@@ -974,6 +977,7 @@ __global__ void __launch_bounds__(K4_THREADS, 2) k4_resolve_order(
     KeyT* __restrict__ kept_key, uint16_t* __restrict__ kept_pos, int* __restrict__ out_counts) {
   extern __shared__ __align__(16) uint8_t smem[];
   __shared__ FrameDesc fd;
+  pdl_wait();
   const int K = cst.top_k, kpad = cst.kpad;
   const size_t uni_b = k4_union_bytes((size_t)K, (size_t)kpad, sizeof(KeyT));
   uint32_t* st32 = reinterpret_cast<uint32_t*>(smem);                  // resolve phase: state, rem, blk bytes
@@ -1187,6 +1191,7 @@ __global__ void __launch_bounds__(K4E_THREADS) k4e_emit(const FrameDesc* __restr
                                                         const KeyT* __restrict__ kept_key, const uint16_t* __restrict__ kept_pos,
                                                         const int* __restrict__ out_counts, Consts cst,
                                                         ffpp_box* __restrict__ out_boxes, uint32_t* __restrict__ hist32) {
+  pdl_wait();
   const int f = blockIdx.y;
   const int r = blockIdx.x * K4E_THREADS + threadIdx.x;
   if (r >= out_counts[f]) return;
@@ -1291,7 +1296,8 @@ __global__ void __launch_bounds__(K5_THREADS, (RT <= K5_PACKED_MAX_RT ? 4 : 2)) 
   constexpr int RB = K5_RB, NW = RB + 2 * RT;
   const int f = blockIdx.y;
   const FrameDesc* fd = &frames[f];
-  if ((int)blockIdx.x >= fd->k5_tiles) return;
+  if ((int)blockIdx.x >= fd->k5_tiles) return;                // the descriptor table is older than the whole run
+  pdl_wait();
   const int gw = fd->gw, gh = fd->gh;
   const int tw = k5_tile_w(gw), th = fd->k5_th;
   int ty = (int)blockIdx.x, tx = 0;
