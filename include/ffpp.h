@@ -57,7 +57,7 @@ typedef struct ffpp_params {
                                   frames in proportion to min(N_f, top_k)); 0 = nms_edges_per_box edges per box       */
   int32_t nms_edges_per_box; /* 0 = 16.  An edge is one unordered pair {a, b} with IoU > iou_thresh; the flock
                                 workloads have 4-9 per box.  The pool is a speed knob, never a correctness limit: a
-                                frame that needs more than its share is resolved by the pool-free overflow kernel
+                                frame that needs more than its share is resolved by the pool-free overflow path of a4
                                 (same result, bounded workspace, slower for that frame)                               */
   int32_t reserved_;
 } ffpp_params;

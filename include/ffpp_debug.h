@@ -20,7 +20,7 @@ extern "C" {
  *   what = 4: a3 work counters of the last run made while       dst HOST int64 [4] = culling-box tests (4 fp32
  *             ffpp_debug_count_work was on                       compares each), exact fp32 IoU evaluations (O5),
  *                                                                suppression edges found, frames that overflowed
- *                                                                their edge-pool share (resolved by the overflow kernel)
+ *                                                                their edge-pool share (resolved pool-free by their a4 CTA)
  *   what = 5: per-frame flag: 1 = the frame took the a3         dst HOST int32 [B]
  *             overflow path in the last run */
 int ffpp_debug_read(ffpp_handle* h, int32_t what, void* dst /*HOST*/, int64_t dst_bytes);

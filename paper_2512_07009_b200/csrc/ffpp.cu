@@ -296,7 +296,7 @@ int launch_all(ffpp_handle* h, const void* raw, int B, cudaStream_t st, ffpp_box
              h->d_sel_box, h->d_sp_box, static_cast<KeyT*>(h->d_sp_key), h->d_cellstart, h->n_sorted(), h->d_hist32,
              reinterpret_cast<uint32_t*>(h->d_hasin), h->sm_count);
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[3], st));
-  // a3 (+ the pool-free overflow path: its CTAs exit at once unless k3 flagged their frame)
+  // a3 (a frame that overflows its share of the edge pool is flagged and resolved pool-free by its a4 CTA)
   {
     const dim3 g3((unsigned)((g.max_nmax + K3_THREADS - 1) / K3_THREADS), (unsigned)B);
     if (g3.x > 0) {
@@ -306,15 +306,13 @@ int launch_all(ffpp_handle* h, const void* raw, int B, cudaStream_t st, ffpp_box
       else
         launch_dep(k3_nms_edges<KeyT, false>, g3, dim3(K3_THREADS), 0, st, frames, h->n_sorted(), h->d_sp_box,
                    static_cast<const KeyT*>(h->d_sp_key), h->d_cellstart, c, h->edge_ctr(), h->d_edges, h->d_hasin, h->frame_err(), h->d_work);
-      launch_dep(k3o_overflow<KeyT>, dim3((unsigned)B), dim3(K3O_THREADS), (size_t)c.kpad, st, frames, h->n_sorted(), h->d_sp_box,
-                 static_cast<const KeyT*>(h->d_sp_key), h->d_cellstart, c, h->edge_ctr(), h->d_hasin, h->frame_err());
     }
   }
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[4], st));
   // a4 (+ a5 histogram)
   launch_dep(k4_resolve_order<KeyT>, dim3((unsigned)B), dim3(K4_THREADS), k4_smem_bytes((size_t)c.top_k, (size_t)c.kpad, sizeof(KeyT)), st,
              frames, h->n_sorted(), h->d_sp_box, static_cast<const KeyT*>(h->d_sp_key), h->edge_ctr(), h->d_edges,
-             reinterpret_cast<const uint32_t*>(h->d_hasin), c, h->sm_count, h->d_k4_scratch,
+             reinterpret_cast<const uint32_t*>(h->d_hasin), h->d_cellstart, h->frame_err(), c, h->sm_count, h->d_k4_scratch,
              static_cast<KeyT*>(h->d_kept_key), h->d_kept_pos, out_counts);
   {
     const dim3 g4e((unsigned)((g.max_nmax + K4E_THREADS - 1) / K4E_THREADS), (unsigned)B);
@@ -351,7 +349,6 @@ int set_kernel_attrs(ffpp_handle* h) {
   FFPP_CUDA(h, cudaFuncSetAttribute(k2_select_bin<kHalf, KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s2));
   const size_t s4 = k4_smem_bytes((size_t)h->p.top_k, (size_t)h->kpad, sizeof(KeyT));
   FFPP_CUDA(h, cudaFuncSetAttribute(k4_resolve_order<KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s4));
-  FFPP_CUDA(h, cudaFuncSetAttribute(k3o_overflow<KeyT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->kpad));
   return FFPP_OK;
 }
 

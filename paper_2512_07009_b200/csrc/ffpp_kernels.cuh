@@ -697,44 +697,27 @@ __global__ void __launch_bounds__(K3_THREADS, 12) k3_nms_edges(const FrameDesc* 
 
 // =====================================================================================================
 // a3/a4 overflow path — a frame whose suppression pairs do not fit its share of the edge pool (k3 raised frame_err[f]).
-// Greedy NMS is the unique fixed point of  kept(a) <=> no kept b before a with IoU(a,b) > thr;  this kernel iterates to
-// it WITHOUT storing pairs: one CTA per flagged frame (all other CTAs exit at once), one state byte per box in shared
-// memory, and per round every undecided box re-examines its partner window (the same cell window as k3, both
+// Greedy NMS is the unique fixed point of  kept(a) <=> no kept b before a with IoU(a,b) > thr;  the frame's a4 CTA
+// iterates to it WITHOUT stored pairs: one state byte per box in shared memory (the same bytes the edge-list fixed
+// point uses), and per round every undecided box re-examines its partner window (the same cell window as k3, both
 // directions this time):
 //     some kept partner before it has IoU > thr          -> removed
 //     no undecided-or-kept partner before it has IoU > thr -> kept
 //     otherwise                                             -> stays undecided.
 // K and R are final, so a decision taken from states another thread is updating in the same round is still right
 // (chaotic iteration); the first undecided box of the order always decides, so the loop ends after at most
-// (longest chain of overlapping boxes with decreasing score) rounds.  Workspace: kpad bytes of shared memory, whatever
-// the input.  The result goes to a4 through the frame's hasin bytes (0 = kept, 3 = removed) with an empty edge list.
+// (longest chain of overlapping boxes with decreasing score) rounds.  Workspace: the state bytes, whatever the input.
 // =====================================================================================================
-constexpr int K3O_THREADS = 1024;
-template <typename KeyT>
-__global__ void __launch_bounds__(K3O_THREADS) k3o_overflow(const FrameDesc* __restrict__ frames, const int* __restrict__ n_sorted,
-                                                            const float4* __restrict__ sp_box,
-                                                            const KeyT* __restrict__ sp_key, const uint16_t* __restrict__ cellstart,
-                                                            Consts cst, int* __restrict__ edge_ctr, uint8_t* __restrict__ hasin,
-                                                            const int* __restrict__ frame_err) {
-  extern __shared__ __align__(16) uint8_t s_state[];          // kpad bytes
-  pdl_wait();
-  const int f = blockIdx.x;
-  if (!frame_err[f]) return;
-  const int n = n_sorted[f];
-  const int tid = threadIdx.x;
-  const FrameDesc* fd = &frames[f];
-  const int cgw = fd->cgw, cgh = fd->cgh, hs = fd->hshift;
-  const int64_t obase = (int64_t)f * cst.kpad;
-  const float4* fbox = sp_box + obase;
-  const KeyT* fkey = sp_key + obase;
-  const uint16_t* cs = cellstart + (int64_t)f * kCellStride;
-  volatile uint8_t* st = s_state;
-  for (int i = tid; i < n; i += K3O_THREADS) st[i] = (uint8_t)ST_U;
-  __syncthreads();
+template <typename KeyT, int kThreads>
+__device__ __forceinline__ void overflow_fixed_point(uint8_t* state, const int n, const FrameDesc& fd, const float4* __restrict__ fbox,
+                                                     const KeyT* __restrict__ fkey, const uint16_t* __restrict__ cs, const Consts& cst,
+                                                     const int tid) {
+  const int cgw = fd.cgw, cgh = fd.cgh, hs = fd.hshift;
+  volatile uint8_t* st = state;
   const float cmx = (float)((cgw << hs) - 1), cmy = (float)((cgh << hs) - 1);
   for (;;) {
     bool undecided = false;
-    for (int p = tid; p < n; p += K3O_THREADS) {
+    for (int p = tid; p < n; p += kThreads) {
       if (st[p] != ST_U) continue;
       const float4 a = fbox[p];
       const KeyT ka = fkey[p];
@@ -764,9 +747,6 @@ __global__ void __launch_bounds__(K3O_THREADS) k3o_overflow(const FrameDesc* __r
     }
     if (!__syncthreads_or(undecided)) break;
   }
-  uint8_t* hz = hasin + obase;
-  for (int i = tid; i < n; i += K3O_THREADS) hz[i] = st[i] == ST_K ? 0 : 3;    // k4: st = hasin ^ 1 -> K (1) / R (2)
-  if (tid == 0) edge_ctr[f] = 0;
 }
 
 // =====================================================================================================
@@ -973,8 +953,9 @@ template <typename KeyT>
 __global__ void __launch_bounds__(K4_THREADS, 2) k4_resolve_order(
     const FrameDesc* __restrict__ frames, const int* __restrict__ n_sorted, const float4* __restrict__ sp_box,
     const KeyT* __restrict__ sp_key, const int* __restrict__ edge_ctr, uint32_t* edges,
-    const uint32_t* __restrict__ hasin, Consts cst, int sm_count, uint8_t* __restrict__ scratch,
-    KeyT* __restrict__ kept_key, uint16_t* __restrict__ kept_pos, int* __restrict__ out_counts) {
+    const uint32_t* __restrict__ hasin, const uint16_t* __restrict__ cellstart, const int* __restrict__ frame_err, Consts cst,
+    int sm_count, uint8_t* __restrict__ scratch, KeyT* __restrict__ kept_key, uint16_t* __restrict__ kept_pos,
+    int* __restrict__ out_counts) {
   extern __shared__ __align__(16) uint8_t smem[];
   __shared__ FrameDesc fd;
   pdl_wait();
@@ -1030,18 +1011,20 @@ __global__ void __launch_bounds__(K4_THREADS, 2) k4_resolve_order(
   if (tid == 0) fd = frames[f];
   const int n = n_sorted[f];
   const int64_t obase = (int64_t)f * kpad;
+  const bool overflow = frame_err[f] != 0;                             // k3 ran out of this frame's share of the edge pool
   {
     const uint32_t* hin = hasin + obase / 4;
     for (int i = tid; i < kpad / 4; i += K4_THREADS) {
-      st32[i] = hin[i] ^ 0x01010101u;                                  // victim of some edge (1) -> U, nobody's victim (0) -> K;
-                                                                       // overflow path: 0 -> K, 3 -> R, with an empty edge list
+      st32[i] = overflow ? 0u : hin[i] ^ 0x01010101u;                  // victim of some edge (1) -> U, nobody's victim (0) -> K;
+                                                                       // overflow path: everybody starts U
       rem32[i] = 0u;
       blk32[i] = 0u;
     }
   }
   __syncthreads();
   FFPP_PHASE(f, 1);
-  const int E = edge_ctr[f];
+  if (overflow) overflow_fixed_point<KeyT, K4_THREADS>(st, n, fd, sp_box + obase, sp_key + obase, cellstart + (int64_t)f * kCellStride, cst, tid);
+  const int E = overflow ? 0 : edge_ctr[f];
   uint32_t* fe = edges + fd.edge_off;
 
   // ---- fixed point over this thread's strided slice of the edge list, compacted in place ----

@@ -182,7 +182,7 @@ def test_wild_box_sizes_against_every_threshold(env, thr):
     raw[twins, :4] = raw[twins[0], :4] * rng.uniform(0.97, 1.03, size=(300, 4))   # a pile of near-identical shapes
     raw[js, 4] = rng.uniform(-1.0, 8.0, size=3000)
     w = W(raw, [[640, 640]], dict(P, dtype="fp32", top_k=2500, iou_thresh=thr))
-    check(env, w)                                        # default pool: whatever does not fit goes through the overflow kernel
+    check(env, w)                                        # default pool: whatever does not fit goes through the overflow path
     if thr in (0.0, 0.5):
         check(env, w, nms_edges_per_box=1300)           # and with room for every pair (at thr ~ 0 the frame-sized boxes touch everything)
 

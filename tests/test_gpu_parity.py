@@ -68,7 +68,7 @@ def test_larger_configs_reduced_batch(torch_cuda, ffpp_mod, oracle_mod, gen_mod,
 
 def test_edge_pool_exhaustion_still_matches_the_oracle(torch_cuda, ffpp_mod, oracle_mod, gen_mod):
     """The suppression-edge pool is a speed knob, not a correctness limit: with one edge per box every frame of a dense
-    batch overflows its share and is resolved by the pool-free overflow kernel — same keep lists, same density."""
+    batch overflows its share and is resolved by the pool-free overflow path — same keep lists, same density."""
     w = gen_mod.make_config(4, B=2)
     pp, out, ref = run_both(torch_cuda, ffpp_mod, oracle_mod, w, nms_edges_per_box=1)
     assert pp.debug_read(5, w.B).all(), "every frame should have taken the overflow path"
