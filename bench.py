@@ -4,8 +4,8 @@ post-processed frames/s and candidates/s at 1 B200; % of roofline per stage).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference]
 
-One "step" = one ffpp_run over one whole batch of the chosen config (all §8(a) rows a0-a6: seven kernel launches
-and one counter memset on one stream).  Default workload: config 5 (ragged 256-frame multi-zone batch, 6 639 360
+One "step" = one ffpp_run over one whole batch of the chosen config (all §8(a) rows a0-a6: seven kernel launches on
+one stream, six of them programmatic dependents of their predecessor).  Default workload: config 5 (ragged 256-frame multi-zone batch, 6 639 360
 candidates, 66.4 MB fp16), the largest single-GPU configuration and the only one that exercises the ragged
 scheduler; the default single-GPU run also measures configs 1-4 briefly and carries them in `configs`.
 Rank r of N generates its own batch (seed offset r): frames are independent, so N GPUs = N x the frames, no
@@ -203,6 +203,26 @@ def reduce_over_ranks(total_ms: float, t_e2e: float, frames: float, cands: float
     u = torch.tensor([frames, cands], dtype=torch.float64, device=device)
     dist.all_reduce(u, op=dist.ReduceOp.SUM)
     return float(t[0]), float(t[1]), float(u[0]), float(u[1])
+
+
+def write_e2e_trace(path: str, step_host, torch):
+    """One ffpp_run_host call under torch.profiler (CUPTI activity records): every copy, memset and kernel with its
+    stream, start and duration, as text.  A diagnostic, never a timing source for the bench line."""
+    from torch.profiler import ProfilerActivity, profile
+    import tempfile
+    with profile(activities=[ProfilerActivity.CUDA]) as prof:
+        step_host()
+        torch.cuda.synchronize()
+    with tempfile.NamedTemporaryFile(suffix=".json") as tf:
+        prof.export_chrome_trace(tf.name)
+        ev = [e for e in json.load(open(tf.name))["traceEvents"] if e.get("ph") == "X" and e.get("cat") in ("kernel", "gpu_memcpy", "gpu_memset")]
+    ev.sort(key=lambda e: e["ts"])
+    t0 = ev[0]["ts"] if ev else 0
+    with open(path, "w") as fh:
+        fh.write("start_us  dur_us  end_us  stream  what  bytes\n")
+        for e in ev:
+            fh.write(f"{e['ts'] - t0:9.1f} {e['dur']:8.1f} {e['ts'] - t0 + e['dur']:9.1f}  s{e['args'].get('stream', '?'):<3} "
+                     f"{e['name'].replace('void ffpp::', '')[:40]:40s} {e['args'].get('bytes', '')}\n")
 
 
 def a3_roofline(work: np.ndarray, ms: float, sm_count: int, sm_mhz: float) -> dict:
@@ -519,6 +539,8 @@ def run_ours(args):
         t_e2e += time.perf_counter() - t0
     torch.cuda.synchronize(); barrier()
     clocks = sampler.stop()
+    if args.e2e_trace and rank == 0:
+        write_e2e_trace(args.e2e_trace, step_host, torch)
     h2d = int(w.raw.nbytes)
     d2h = int(4 * B + 4 * cells + 24 * int(kept.sum()))
     # PCIe floor of the same transfers: pinned H2D of the raw buffer and pinned D2H of the density, each alone
@@ -649,7 +671,7 @@ def run_ours(args):
                     "pcie_h2d_GB/s": h2d / (h2d_ms * 1e-3) / 1e9, "frac_of_pcie_floor": max(h2d_ms, d2h_ms) / e2e_ms,
                     "api": "ffpp_run_host (pinned host buffers, copies + sync inside the timed region)"},
             "gpu_launches": ffpp.LAUNCHES_PER_RUN * K,
-            "launches_per_step": {"kernels": ffpp.LAUNCHES_PER_RUN, "memsets": 1, "descriptor_uploads": 0},
+            "launches_per_step": {"kernels": ffpp.LAUNCHES_PER_RUN, "memsets": 0, "descriptor_uploads": 0},
             "roofline": roofline,
             "step_roofline": step_roofline,
             "stages": stages,
@@ -680,6 +702,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-other-configs", action="store_true", help="skip the short measurements of the other four configs")
     ap.add_argument("--no-next", action="store_true", help="skip the measurements of the SURVEY 8(f) rows f1-f4")
+    ap.add_argument("--e2e-trace", default=None, metavar="FILE",
+                    help="also write a text timeline (copies and kernels per stream, from torch.profiler / CUPTI) of one ffpp_run_host call")
     args = ap.parse_args()
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         return respawn_under_torchrun(args)

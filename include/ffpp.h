@@ -101,8 +101,9 @@ int ffpp_run(ffpp_handle* h, const void* raw /*DEVICE*/, int32_t B, const int32_
 /* The same path with HOST buffers (the call a user without device buffers makes): copies raw host->device,
  * runs, copies the three outputs device->host through the handle's own staging, and synchronises `stream`
  * before returning.  raw / out_* are HOST pointers (pinned memory makes the copies asynchronous DMA; a pinned
- * out_boxes is written by one kernel through its device alias).  Batches of >= 16 MB and >= 8 frames are cut by
- * bytes into up to 4 runs of whole frames (frames are independent) so that the upload of the next run and the
+ * out_boxes is written by one kernel through its device alias).  Batches of >= 16 MB and >= 12 frames are cut by
+ * bytes into up to 6 runs of whole frames (frames are independent; consecutive runs alternate between two compute
+ * streams and two workspaces, the second one created on the first such call) so that the upload of the next run and the
  * download of the previous one, on two internal copy streams, overlap the kernels of the current run on
  * `stream` (the D2H copy + CPU post-processing the paper blames; L308-310: streams as the remedy). */
 int ffpp_run_host(ffpp_handle* h, const void* raw /*HOST*/, int32_t B, const int32_t* N_per_frame /*HOST*/,

@@ -32,12 +32,12 @@ FFPP_OK, FFPP_EINVAL, FFPP_ECAPACITY, FFPP_ECUDA, FFPP_ENOMEM = 0, -1, -2, -3, -
 NUM_STAGES = 6
 STAGE_NAMES = ["a0_schedule", "a1_threshold_compact", "a2_select_decode_bin", "a3_nms_pairs", "a4_nms_resolve_emit", "a5a6_density"]
 
-STAGE_KERNELS = {"a0_schedule": "host scheduler + memset", "a1_threshold_compact": "k1_threshold_compact",
+STAGE_KERNELS = {"a0_schedule": "host scheduler + k0_clear", "a1_threshold_compact": "k1_threshold_compact",
                  "a2_select_decode_bin": "k2_select_bin", "a3_nms_pairs": "k3_nms_edges",
                  "a4_nms_resolve_emit": "k4_resolve_order + k4e_emit", "a5a6_density": "k5_density"}
-# kernel launches of one ffpp_run (k1, k2, k3, k4, k4e, k5); plus one counter memset and, on first sight of a
+# kernel launches of one ffpp_run (k0_clear, k1, k2, k3, k4, k4e, k5); no memset; on first sight of a
 # batch geometry, one descriptor upload
-LAUNCHES_PER_RUN = 6
+LAUNCHES_PER_RUN = 7
 
 # fp32 instructions per IoU pair of the all-pairs bitmask method (4 min/max, 2 sub, 2 clamp, 1 mul, area
 # add/sub, divide-or-multiply + compare = 12-16; 15 taken).  bench.py divides the fp32 lane rate by this to get the

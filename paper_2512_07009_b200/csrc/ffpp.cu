@@ -91,7 +91,9 @@ struct ffpp_handle {
   int* d_out_counts = nullptr;
   float* d_out_density = nullptr;
   cudaStream_t s_h2d = nullptr, s_d2h = nullptr;     // copy streams of the chunked host path (created on first use)
-  static constexpr int kHostChunks = 4;
+  cudaStream_t s_run2 = nullptr;                     // second compute stream of the chunked host path
+  ffpp_handle* twin = nullptr;                       // second workspace: odd runs of the chunked host path go through it
+  static constexpr int kHostChunks = 6;
   cudaEvent_t ev_up[kHostChunks] = {}, ev_run[kHostChunks] = {};
   // SURVEY §8(f) f1-f3 (ffpp_next.cuh): cached grid tables of f1 / f2 and the component-labelling scratch (grown on demand)
   struct NextGeo {
@@ -285,9 +287,9 @@ int launch_all(ffpp_handle* h, const void* raw, int B, cudaStream_t st, ffpp_box
     const int64_t nchunks = (g.total_cand * row + K1_CHUNK_BYTES - 1) / K1_CHUNK_BYTES;
     int64_t grid = (int64_t)h->sm_count * K1_CTAS_PER_SM;
     if (grid > nchunks) grid = nchunks;
-    k1_threshold_compact<kHalf, KeyT><<<(unsigned)grid, K1_THREADS, K1_STAGES * K1_CHUNK_BYTES, st>>>(
-        static_cast<const uint8_t*>(raw), g.total_cand, B, coff, reinterpret_cast<const int32_t*>(g.d_meta + h->ml.block_frame_off),
-        c.logit_thr, static_cast<KeyT*>(h->d_surv_keys), h->surv_cnt());
+    launch_dep(k1_threshold_compact<kHalf, KeyT>, dim3((unsigned)grid), dim3(K1_THREADS), (size_t)(K1_STAGES * K1_CHUNK_BYTES), st,
+               static_cast<const uint8_t*>(raw), g.total_cand, B, coff, reinterpret_cast<const int32_t*>(g.d_meta + h->ml.block_frame_off),
+               c.logit_thr, static_cast<KeyT*>(h->d_surv_keys), h->surv_cnt());
   }
   if (tm) FFPP_CUDA(h, cudaEventRecord(h->ev[2], st));
   // a2 (+ clears the a5 histogram)
@@ -512,8 +514,7 @@ int ffpp_run(ffpp_handle* h, const void* raw, int32_t B, const int32_t* N_per_fr
   if (h->timing) FFPP_CUDA(h, cudaEventRecord(h->ev[0], st));
   int rc = schedule(h, B, N_per_frame, frame_dims, st);
   if (rc != FFPP_OK) return rc;
-  FFPP_CUDA(h, cudaMemsetAsync(h->d_counters, 0, sizeof(int) * (3 + kCntStride) * (size_t)h->p.max_frames, st));
-  if (h->count_work) FFPP_CUDA(h, cudaMemsetAsync(h->d_work, 0, 4 * sizeof(unsigned long long), st));
+  k0_clear<<<(unsigned)(((3 + kCntStride) * B + 255) / 256), 256, 0, st>>>(h->d_counters, h->p.max_frames, B, h->count_work ? h->d_work : nullptr);
   if (h->half && h->key_bytes == 4) return launch_all<true, uint32_t>(h, raw, B, st, out_boxes, out_counts, out_density);
   if (h->half) return launch_all<true, uint64_t>(h, raw, B, st, out_boxes, out_counts, out_density);
   return launch_all<false, uint64_t>(h, raw, B, st, out_boxes, out_counts, out_density);
@@ -566,19 +567,22 @@ int ffpp_run_host(ffpp_handle* h, const void* raw, int32_t B, const int32_t* N_p
   }
   // Frames are independent, so a large batch is cut BY BYTES into up to kHostChunks runs of whole frames: the upload of
   // run i+1 (copy stream) and the download of run i-1 (second copy stream) overlap the kernels of run i on `stream`.
-  // A run starts where the raw byte offset is a multiple of 16 (ffpp_run's alignment rule).  Four equal runs measured
-  // best on config 5 (1.61 ms against 2.06 with eight, 1.75 with three, 2.10 with one): a run's kernel chain costs
-  // 160-280 us however few frames it holds (one CTA per frame in a2 / a4), so more runs than four make the batch
-  // kernel-bound instead of PCIe-bound, and unequal shares only move that time around (profiles/r2_e2e_timeline.md).
+  // A run starts where the raw byte offset is a multiple of 16 (ffpp_run's alignment rule).  A run's kernel chain costs
+  // ~160 us however few frames it holds (one CTA per frame in a2 / a4), so consecutive runs alternate between two
+  // compute streams and two workspaces (this handle's and its twin's): two chains are in flight and the batch stays
+  // PCIe-bound.  What is left after the last upload is one chain + its download; six runs with shrinking shares
+  // measured best on config 5 (1.56 ms; four equal runs on one stream 1.61, eight 2.06, one 2.10; the H2D copies
+  // alone take 1.33 ms while downloads run beside them; profiles/r2_e2e_timeline.md).
   constexpr int kHostChunks = ffpp_handle::kHostChunks;
-  static const int kShare[kHostChunks] = {5, 5, 5, 5};                        // of 20: relative raw bytes of the runs
+  static const int kShare[kHostChunks] = {4, 4, 4, 3, 3, 2};                  // of 20: relative raw bytes of the runs
+  const int nshare = kHostChunks;
   const size_t row = 5 * esz;
   std::vector<int> cut{0};                                          // first frame of every run, then B
   if (B >= 2 * kHostChunks && (size_t)cand * row >= ((size_t)16 << 20)) {
     int64_t acc = 0, want = 0;
     int next = 0;
     want = cand * kShare[0] / 20;
-    for (int f = 0; f < B && next + 1 < kHostChunks; ++f) {
+    for (int f = 0; f < B && next + 1 < nshare; ++f) {
       if (f > cut.back() && acc * (int64_t)row % 16 == 0 && acc >= want) {
         cut.push_back(f); ++next;
         int sh = 0;
@@ -593,15 +597,22 @@ int ffpp_run_host(ffpp_handle* h, const void* raw, int32_t B, const int32_t* N_p
   if (C > 1 && !h->s_h2d) {
     FFPP_CUDA(h, cudaStreamCreateWithFlags(&h->s_h2d, cudaStreamNonBlocking));
     FFPP_CUDA(h, cudaStreamCreateWithFlags(&h->s_d2h, cudaStreamNonBlocking));
+    FFPP_CUDA(h, cudaStreamCreateWithFlags(&h->s_run2, cudaStreamNonBlocking));
     for (int i = 0; i < kHostChunks; ++i) {
       FFPP_CUDA(h, cudaEventCreateWithFlags(&h->ev_up[i], cudaEventDisableTiming));
       FFPP_CUDA(h, cudaEventCreateWithFlags(&h->ev_run[i], cudaEventDisableTiming));
     }
   }
+  if (C > 1 && !h->twin) {                                          // the second workspace (same parameters), first chunked call only
+    ffpp_params tp = h->p;
+    const int trc = ffpp_create(&tp, &h->twin);
+    if (trc != FFPP_OK) { h->twin = nullptr; return fail(h, trc, std::string("host path: second workspace: ") + ffpp_last_error(nullptr)); }
+  }
   cudaStream_t s_up = C > 1 ? h->s_h2d : st, s_dn = C > 1 ? h->s_d2h : st;
   if (C > 1) {                                                      // the copy streams start after what is already on `stream`
     FFPP_CUDA(h, cudaEventRecord(h->ev_run[0], st));
     FFPP_CUDA(h, cudaStreamWaitEvent(s_up, h->ev_run[0], 0));
+    FFPP_CUDA(h, cudaStreamWaitEvent(h->s_run2, h->ev_run[0], 0));
   }
   std::vector<int64_t> c_off((size_t)C + 1, 0), d_off((size_t)C + 1, 0);
   for (int i = 0; i < C; ++i) {
@@ -623,12 +634,20 @@ int ffpp_run_host(ffpp_handle* h, const void* raw, int32_t B, const int32_t* N_p
   }
   for (int i = 0; i < C; ++i) {
     const int f0 = cut[(size_t)i], Bi = cut[(size_t)i + 1] - f0;
-    if (C > 1) FFPP_CUDA(h, cudaStreamWaitEvent(st, h->ev_up[i], 0));
-    const int rc = ffpp_run(h, d_in8 + (size_t)c_off[(size_t)i] * row, Bi, N_per_frame + f0, frame_dims + 2 * f0, stream,
+    // two kernel chains in flight: even runs on `stream` with this handle's workspace, odd runs on the second compute
+    // stream with the twin's (a run's chain is latency-bound: one CTA per frame in a2 / a4, so two chains share the SMs well)
+    ffpp_handle* hr = (C > 1 && (i & 1)) ? h->twin : h;
+    cudaStream_t sr = (C > 1 && (i & 1)) ? h->s_run2 : st;
+    if (C > 1) FFPP_CUDA(h, cudaStreamWaitEvent(sr, h->ev_up[i], 0));
+    const int rc = ffpp_run(hr, d_in8 + (size_t)c_off[(size_t)i] * row, Bi, N_per_frame + f0, frame_dims + 2 * f0, sr,
                             h->d_out_boxes + (size_t)f0 * K, h->d_out_counts + f0, h->d_out_density + d_off[(size_t)i]);
-    if (rc != FFPP_OK) { cudaStreamSynchronize(s_up); cudaStreamSynchronize(st); cudaStreamSynchronize(s_dn); return rc; }
+    if (rc != FFPP_OK) {
+      if (hr != h) h->err = hr->err;
+      cudaStreamSynchronize(s_up); cudaStreamSynchronize(st); if (C > 1) cudaStreamSynchronize(h->s_run2); cudaStreamSynchronize(s_dn);
+      return rc;
+    }
     if (C > 1) {
-      FFPP_CUDA(h, cudaEventRecord(h->ev_run[i], st));
+      FFPP_CUDA(h, cudaEventRecord(h->ev_run[i], sr));
       FFPP_CUDA(h, cudaStreamWaitEvent(s_dn, h->ev_run[i], 0));
     }
     if (alias) {
@@ -640,6 +659,7 @@ int ffpp_run_host(ffpp_handle* h, const void* raw, int32_t B, const int32_t* N_p
                                  sizeof(float) * (size_t)(d_off[(size_t)i + 1] - d_off[(size_t)i]), cudaMemcpyDeviceToHost, s_dn));
   }
   FFPP_CUDA(h, cudaStreamSynchronize(s_dn));
+  if (C > 1) FFPP_CUDA(h, cudaStreamSynchronize(h->s_run2));
   FFPP_CUDA(h, cudaStreamSynchronize(st));
   if (!alias) {
     for (int f = 0; f < B; ++f)
@@ -661,6 +681,8 @@ int ffpp_destroy(ffpp_handle* h) {
   cudaFree(h->d_in); cudaFree(h->d_out_boxes); cudaFree(h->d_out_counts); cudaFree(h->d_out_density);
   for (int sl = 0; sl < ffpp_handle::kNextSlots; ++sl) cudaFree(h->ngeo[sl].d_tab);
   cudaFree(h->d_ccl_aux); cudaFree(h->d_ccl_sums); cudaFree(h->d_ccl_blk); cudaFree(h->d_ent_part);
+  if (h->twin) ffpp_destroy(h->twin);
+  if (h->s_run2) cudaStreamDestroy(h->s_run2);
   if (h->s_h2d) cudaStreamDestroy(h->s_h2d);
   if (h->s_d2h) cudaStreamDestroy(h->s_d2h);
   for (int i = 0; i < ffpp_handle::kHostChunks; ++i) { if (h->ev_up[i]) cudaEventDestroy(h->ev_up[i]); if (h->ev_run[i]) cudaEventDestroy(h->ev_run[i]); }

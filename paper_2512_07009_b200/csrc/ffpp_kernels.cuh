@@ -18,6 +18,17 @@ namespace ffpp {
 // here: only the <= top_k rows that survive the sort are decoded, in the a2 epilogue.
 // There is no __syncthreads in the steady state; the frame offset table sits in shared memory.
 // =====================================================================================================
+// a0 on the device: the per-frame counters of a run (top-K counts, edge counts, overflow flags, one line per frame of
+// survivor counts) are cleared by a kernel, not by cudaMemsetAsync: a memset node was seen to queue behind the DMA
+// traffic of the chunked host path for tens of microseconds (profiles/r2_e2e_timeline.md), a kernel is not, and a1 can
+// be its programmatic dependent.
+__global__ void __launch_bounds__(256) k0_clear(int* __restrict__ counters, int max_frames, int B, unsigned long long* __restrict__ work) {
+  const int i = blockIdx.x * 256 + threadIdx.x;
+  if (i < 3 * B) counters[(i / B) * max_frames + (i % B)] = 0;                 // n_sorted | edge_ctr | frame_err
+  else if (i < (3 + kCntStride) * B) counters[3 * max_frames + (i - 3 * B)] = 0;   // survivor counters, kCntStride ints per frame
+  if (work && i < 4) work[i] = 0ull;
+}
+
 constexpr int K1_CONSUMERS = 8;
 constexpr int K1_THREADS = 32 * (K1_CONSUMERS + 1);
 constexpr int K1_CHUNK_BYTES = 20480;   // multiple of lcm(16, 10, 20) = 80 and of 8 warps x 32 lanes rows
@@ -63,6 +74,7 @@ __global__ void __launch_bounds__(K1_THREADS) k1_threshold_compact(const uint8_t
     for (int s = 0; s < K1_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], K1_CONSUMERS); }
     mbar_fence_init();
   }
+  pdl_wait();                                                  // the counters are being cleared by k0_clear
   const bool coff_in_smem = B <= K1_SMEM_FRAMES;
   if (coff_in_smem)
     for (int i = tid; i <= B; i += K1_THREADS) s_coff[i] = cand_off[i];
