@@ -990,7 +990,7 @@ __global__ void __launch_bounds__(K4_THREADS, 2) k4_resolve_order(
   // first, so which SMs stay single is approximate).  The frames are ranked by an estimate of their a4 time (edges,
   // boxes, and the kept count the edge count implies): the 2S-B longest go to the CTAs expected to stay alone, the next
   // longest are paired with the shortest.  What matters most is that long frames never pair with long ones.
-  __shared__ int s_w[K4_MAXPERM];
+  __shared__ __align__(16) int s_w[K4_MAXPERM];
   __shared__ int s_frame;
   {
     const int B = (int)gridDim.x, S = sm_count, i = (int)blockIdx.x;
@@ -1009,12 +1009,31 @@ __global__ void __launch_bounds__(K4_THREADS, 2) k4_resolve_order(
       else if (i >= S - alone) want = i - (S - alone);             // alone on its SM: the longest frames
       else want = alone + i;                                       // first CTA of a shared SM
       if (B >= 2 * S) want = i < S ? i : (i < 2 * S ? B - 1 - (i - S) : S + (i - 2 * S));
-      for (int g = tid; g < B; g += K4_THREADS) {
+      // rank of frame g = frames that weigh more (ties: lower index first); the comparisons of one frame are split over
+      // K4_THREADS / Bp threads, four weights per shared load
+      const int Bp = (B + 3) & ~3;
+      for (int g = tid; g < Bp; g += K4_THREADS) if (g >= B) s_w[g] = INT_MIN;   // padding never outranks a frame
+      int* s_rank = reinterpret_cast<int*>(smem);                                // the dynamic area is free until the frame is known
+      for (int g = tid; g < B; g += K4_THREADS) s_rank[g] = 0;
+      __syncthreads();
+      const int parts = B <= K4_THREADS / 2 ? K4_THREADS / B : 1;               // threads per frame
+      const int g0 = tid / parts, part = tid - g0 * parts;
+      for (int g = g0; g < B; g += K4_THREADS / parts) {
         const int wg = s_w[g];
+        const int q4 = Bp / 4, qa = q4 * part / parts, qb = q4 * (part + 1) / parts;
         int rank = 0;
-        for (int h = 0; h < B; ++h) { const int wh = s_w[h]; rank += (wh > wg) | ((wh == wg) & (h < g)); }
-        if (rank == want) s_frame = g;
+        for (int q = qa; q < qb; ++q) {
+          const int4 v = reinterpret_cast<const int4*>(s_w)[q];
+          const int h = 4 * q;
+          rank += (v.x > wg) | ((v.x == wg) & (h < g));
+          rank += (v.y > wg) | ((v.y == wg) & (h + 1 < g));
+          rank += (v.z > wg) | ((v.z == wg) & (h + 2 < g));
+          rank += (v.w > wg) | ((v.w == wg) & (h + 3 < g));
+        }
+        if (parts > 1) atomicAdd(&s_rank[g], rank); else s_rank[g] = rank;
       }
+      __syncthreads();
+      for (int g = tid; g < B; g += K4_THREADS) if (s_rank[g] == want) s_frame = g;
     }
     __syncthreads();
   }
@@ -1045,35 +1064,61 @@ __global__ void __launch_bounds__(K4_THREADS, 2) k4_resolve_order(
 #ifdef FFPP_PROFILE_PHASES
   int round_ = 0;
 #endif
-  bool first = true;                       // round 1 drops nothing: every victim is still U, so it only sets flags
+  uint32_t* const fmine = fe + tid;            // this thread's k-th edge sits at fmine[k * K4_THREADS]
+  bool first = true;
   for (;;) {
-    int w = 0;
-    uint32_t nx[K4_UNROLL];
+    if (first) {
+      // round 1: every victim is still undecided and no box is removed yet, so an edge only needs its suppressor's
+      // state (kept -> the victim is removed, undecided -> the victim is blocked); nothing is dropped, nothing written back
+      const uint32_t* p = fmine;
+      int k0 = 0;
+      for (; k0 + K4_UNROLL <= mine; k0 += K4_UNROLL, p += K4_UNROLL * K4_THREADS) {
+        uint32_t ed[K4_UNROLL], ss[K4_UNROLL];
 #pragma unroll
-    for (int u = 0; u < K4_UNROLL; ++u) nx[u] = u < mine ? fe[tid + u * K4_THREADS] : 0u;
-    for (int k0 = 0; k0 < mine; k0 += K4_UNROLL) {
-      uint32_t ed[K4_UNROLL], sv[K4_UNROLL], ss[K4_UNROLL];
+        for (int u = 0; u < K4_UNROLL; ++u) ed[u] = p[u * K4_THREADS];
 #pragma unroll
-      for (int u = 0; u < K4_UNROLL; ++u) ed[u] = nx[u];
+        for (int u = 0; u < K4_UNROLL; ++u) ss[u] = st[ed[u] & 0xFFFFu];
 #pragma unroll
-      for (int u = 0; u < K4_UNROLL; ++u)     // next batch: slots beyond anything this batch can write
-        nx[u] = k0 + K4_UNROLL + u < mine ? fe[tid + (k0 + K4_UNROLL + u) * K4_THREADS] : 0u;
+        for (int u = 0; u < K4_UNROLL; ++u) (ss[u] == ST_K ? rem : blk)[ed[u] >> 16] = 1;
+      }
+      for (; k0 < mine; ++k0, p += K4_THREADS) {
+        const uint32_t ed = *p;
+        (st[ed & 0xFFFFu] == ST_K ? rem : blk)[ed >> 16] = 1;
+      }
+    } else {
+      int w = 0;
+      const uint32_t* p = fmine;
+      uint32_t* q = fmine;
+      int k0 = 0;
+      for (; k0 + K4_UNROLL <= mine; k0 += K4_UNROLL, p += K4_UNROLL * K4_THREADS) {
+        uint32_t ed[K4_UNROLL], sv[K4_UNROLL], ss[K4_UNROLL];
 #pragma unroll
-      for (int u = 0; u < K4_UNROLL; ++u) { sv[u] = st[ed[u] >> 16]; ss[u] = st[ed[u] & 0xFFFFu]; }
+        for (int u = 0; u < K4_UNROLL; ++u) ed[u] = p[u * K4_THREADS];      // all loads of the batch before its first store
 #pragma unroll
-      for (int u = 0; u < K4_UNROLL; ++u) {
-        if (k0 + u < mine && sv[u] == ST_U) {
-          const uint32_t v = ed[u] >> 16;
-          if (ss[u] == ST_K) {
-            rem[v] = 1;
-          } else if (ss[u] == ST_U) {
-            blk[v] = 1;
-            if (!first) { fe[tid + w * K4_THREADS] = ed[u]; ++w; }
+        for (int u = 0; u < K4_UNROLL; ++u) { sv[u] = st[ed[u] >> 16]; ss[u] = st[ed[u] & 0xFFFFu]; }
+#pragma unroll
+        for (int u = 0; u < K4_UNROLL; ++u) {
+          if (sv[u] == ST_U) {
+            const uint32_t v = ed[u] >> 16;
+            if (ss[u] == ST_K) {
+              rem[v] = 1;
+            } else if (ss[u] == ST_U) {
+              blk[v] = 1;
+              *q = ed[u]; q += K4_THREADS; ++w;                           // slots at or before the ones this batch read
+            }
           }
         }
       }
+      for (; k0 < mine; ++k0, p += K4_THREADS) {
+        const uint32_t ed = *p;
+        if (st[ed >> 16] == ST_U) {
+          const uint32_t v = ed >> 16, sst = st[ed & 0xFFFFu];
+          if (sst == ST_K) rem[v] = 1;
+          else if (sst == ST_U) { blk[v] = 1; *q = ed; q += K4_THREADS; ++w; }
+        }
+      }
+      mine = w;
     }
-    if (!first) mine = w;
     first = false;
     __syncthreads();
     for (int i = tid; i < nw; i += K4_THREADS) {

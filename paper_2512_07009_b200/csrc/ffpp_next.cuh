@@ -40,6 +40,7 @@ __device__ __forceinline__ float load_prob(const __half* p, const int64_t i) { r
 //   kc_final   mass = sum (f1) or sum / area (f3: mean probability)
 // =====================================================================================================
 constexpr int KC_THREADS = 256;
+constexpr int KC_PER = 1;                         // 256-pixel steps per CTA of the per-pixel kernels (a step = 32 consecutive pixels per warp)
 constexpr int KC_RANK_THREADS = 1024;
 constexpr int KC_RANK_PER = 4;                    // consecutive pixels per thread per step of kc_rank
 constexpr double KC_FIX = 1099511627776.0;        // 2^40
@@ -49,9 +50,11 @@ __global__ void __launch_bounds__(KC_THREADS) kc_init(const T* __restrict__ src,
                                                       float thr, int32_t* __restrict__ labels, int32_t* __restrict__ aux) {
   const ImgDesc d = img_desc(tab, blockIdx.y, w0, h0);
   const int n = d.w * d.h;
-  const int i = blockIdx.x * KC_THREADS + threadIdx.x;
-  if (blockIdx.x * KC_THREADS >= n) return;
   const int lane = threadIdx.x & 31;
+  for (int e = 0; e < KC_PER; ++e) {
+  const int base = (blockIdx.x * KC_PER + e) * KC_THREADS;
+  if (base >= n) break;
+  const int i = base + threadIdx.x;
   const bool valid = i < n;
   const bool fg = valid && load_prob(src, d.off + i) > thr;
   // horizontal runs inside the warp's 32 consecutive pixels start labelled with the run's first pixel: the unions
@@ -63,6 +66,7 @@ __global__ void __launch_bounds__(KC_THREADS) kc_init(const T* __restrict__ src,
   if (valid) {
     labels[d.off + i] = fg ? i - (lane - first) : -1;
     aux[d.off + i] = 0;
+  }
   }
 }
 
@@ -92,18 +96,20 @@ __device__ __forceinline__ void cc_unite(int32_t* L, int a, int b) {
 __global__ void __launch_bounds__(KC_THREADS) kc_merge(const ImgDesc* __restrict__ tab, int w0, int h0, int conn, int32_t* __restrict__ labels) {
   const ImgDesc d = img_desc(tab, blockIdx.y, w0, h0);
   const int w = d.w, n = d.w * d.h;
-  const int i = blockIdx.x * KC_THREADS + threadIdx.x;
-  if (blockIdx.x * KC_THREADS >= n) return;
   const int lane = threadIdx.x & 31;
   int32_t* L = labels + d.off;
+  for (int e = 0; e < KC_PER; ++e) {
+  const int base = (blockIdx.x * KC_PER + e) * KC_THREADS;
+  if (base >= n) break;
+  const int i = base + threadIdx.x;
   const bool valid = i < n;
   const bool fg = valid && L[i] >= 0;                        // foreground never changes: label >= 0
   const uint32_t bits = __ballot_sync(0xffffffffu, fg);
-  if (!fg) return;
+  if (!fg) continue;
   const int y = i / w, x = i - y * w;
   const bool left = x > 0 && (lane > 0 ? ((bits >> (lane - 1)) & 1u) != 0 : L[i - 1] >= 0);
   if (lane == 0 && left) cc_unite(L, i, i - 1);              // the run continues from the previous warp
-  if (y == 0) return;
+  if (y == 0) continue;
   const bool up = L[i - w] >= 0;
   const bool ul = x > 0 && L[i - w - 1] >= 0;
   if (up) {
@@ -115,21 +121,23 @@ __global__ void __launch_bounds__(KC_THREADS) kc_merge(const ImgDesc* __restrict
       if (!right) cc_unite(L, i, i - w + 1);
     }
   }
+  }
 }
 
 __global__ void __launch_bounds__(KC_THREADS) kc_flatten(const ImgDesc* __restrict__ tab, int w0, int h0, int32_t* __restrict__ labels,
                                                          int32_t* __restrict__ aux) {
   const ImgDesc d = img_desc(tab, blockIdx.y, w0, h0);
   const int n = d.w * d.h;
-  const int i = blockIdx.x * KC_THREADS + threadIdx.x;
-  if (i >= n) return;
   int32_t* L = labels + d.off;
-  if (L[i] < 0) return;
-  const int r = cc_find(L, i);
-  if (r != i) L[i] = r;                                      // a chain through i that another thread is walking still ends at r
-  // area: lanes of the warp that found the same root count together (runs of one component are the common case)
-  const uint32_t peers = __match_any_sync(__activemask(), r);
-  if ((int)(__ffs(peers) - 1) == (int)(threadIdx.x & 31)) atomicAdd(&aux[d.off + r], __popc(peers));
+  for (int e = 0; e < KC_PER; ++e) {
+    const int i = (blockIdx.x * KC_PER + e) * KC_THREADS + threadIdx.x;
+    if (i >= n || L[i] < 0) continue;
+    const int r = cc_find(L, i);
+    if (r != i) L[i] = r;                                    // a chain through i that another thread is walking still ends at r
+    // area: lanes of the warp that found the same root count together (runs of one component are the common case)
+    const uint32_t peers = __match_any_sync(__activemask(), r);
+    if ((int)(__ffs(peers) - 1) == (int)(threadIdx.x & 31)) atomicAdd(&aux[d.off + r], __popc(peers));
+  }
 }
 
 // Ordered compaction of the roots with area >= min_area into the table (ascending label), in three launches so that a
@@ -238,7 +246,12 @@ __global__ void __launch_bounds__(KC_THREADS) kc_stats(const T* __restrict__ src
   const int img = blockIdx.y;
   const ImgDesc d = img_desc(tab, img, w0, h0);
   const int w = d.w, n = d.w * d.h;
-  const int i = blockIdx.x * KC_THREADS + threadIdx.x;
+  ffpp_region* table = out + (int64_t)img * max_out;
+  unsigned long long* sm = sums + (int64_t)img * max_out;
+  for (int e = 0; e < KC_PER; ++e) {
+  const int base = (blockIdx.x * KC_PER + e) * KC_THREADS;
+  if (base >= n) break;
+  const int i = base + threadIdx.x;
   int k = -1;
   int x = 0, y = 0;
   unsigned long long fx = 0ull;
@@ -251,9 +264,7 @@ __global__ void __launch_bounds__(KC_THREADS) kc_stats(const T* __restrict__ src
     }
   }
   const uint32_t act = __ballot_sync(0xffffffffu, k >= 0);
-  if (act == 0) return;
-  ffpp_region* table = out + (int64_t)img * max_out;
-  unsigned long long* sm = sums + (int64_t)img * max_out;
+  if (act == 0) continue;
   const int k0 = __shfl_sync(0xffffffffu, k, __ffs(act) - 1);
   if (__all_sync(0xffffffffu, k < 0 || k == k0)) {           // one component in this warp: reduce, then one set of atomics
     int x0 = k >= 0 ? x : INT_MAX, x1 = k >= 0 ? x : -1, y0 = k >= 0 ? y : INT_MAX, y1 = k >= 0 ? y : -1;
@@ -272,6 +283,7 @@ __global__ void __launch_bounds__(KC_THREADS) kc_stats(const T* __restrict__ src
     atomicMin(&table[k].x0, x); atomicMax(&table[k].x1, x);
     atomicMin(&table[k].y0, y); atomicMax(&table[k].y1, y);
     atomicAdd(&sm[k], fx);
+  }
   }
 }
 
@@ -398,12 +410,14 @@ __global__ void __launch_bounds__(KD_THREADS) kd_exact(const ffpp_box* __restric
     __syncthreads();
     for (int k = 0; k < total; ++k) {
       const float2 q = s_uv[k];
+      const float dy0 = __fsub_rn(yc0, q.y), dy1 = __fsub_rn(yc1, q.y);
+      const bool in0 = fabsf(dy0) <= Rf, in1 = fabsf(dy1) <= Rf;
+      if (!(in0 | in1)) continue;                            // warp-uniform: a warp is one row of the tile (and the row 8 below)
       const float dx = __fsub_rn(xc, q.x);
       if (!(fabsf(dx) <= Rf)) continue;
-      const float dy0 = __fsub_rn(yc0, q.y), dy1 = __fsub_rn(yc1, q.y);
       const float dx2 = dx * dx;
-      if (fabsf(dy0) <= Rf) acc0 += expf((dx2 + dy0 * dy0) * neg_inv_2s2) * inv_z2;
-      if (fabsf(dy1) <= Rf) acc1 += expf((dx2 + dy1 * dy1) * neg_inv_2s2) * inv_z2;
+      if (in0) acc0 += expf((dx2 + dy0 * dy0) * neg_inv_2s2) * inv_z2;
+      if (in1) acc1 += expf((dx2 + dy1 * dy1) * neg_inv_2s2) * inv_z2;
     }
     __syncthreads();
   }
@@ -560,7 +574,7 @@ template <typename T>
 int run_ccl(ffpp_handle* h, const T* src, const ffpp::ImgDesc* tab, int B, int w0, int h0, int max_px, float thr, int conn, int min_area,
             int max_out, int mean, cudaStream_t st, int32_t* labels, ffpp_region* out, int32_t* counts) {
   using namespace ffpp;
-  const dim3 g((unsigned)((max_px + KC_THREADS - 1) / KC_THREADS), (unsigned)B);
+  const dim3 g((unsigned)((max_px + KC_THREADS * KC_PER - 1) / (KC_THREADS * KC_PER)), (unsigned)B);
   kc_init<T><<<g, KC_THREADS, 0, st>>>(src, tab, w0, h0, thr, labels, h->d_ccl_aux);
   kc_merge<<<g, KC_THREADS, 0, st>>>(tab, w0, h0, conn, labels);
   kc_flatten<<<g, KC_THREADS, 0, st>>>(tab, w0, h0, labels, h->d_ccl_aux);
