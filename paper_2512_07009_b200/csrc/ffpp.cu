@@ -809,6 +809,10 @@ int ffpp_debug_phases(unsigned long long* dst, int frames) {
   cudaDeviceSynchronize();
   return (int)cudaMemcpyFromSymbol(dst, ffpp::g_phase, sizeof(unsigned long long) * 16 * (size_t)frames);
 }
+int ffpp_debug_phases2(unsigned long long* dst, int frames) {
+  cudaDeviceSynchronize();
+  return (int)cudaMemcpyFromSymbol(dst, ffpp::g_phase2, sizeof(unsigned long long) * 16 * (size_t)frames);
+}
 #endif
 
 }  // extern "C"

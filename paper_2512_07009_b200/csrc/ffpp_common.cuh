@@ -56,9 +56,12 @@ struct Consts {
 #ifdef FFPP_PROFILE_PHASES
 __device__ unsigned long long g_phase[4096][16];
 __device__ __forceinline__ unsigned long long gtimer() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+__device__ unsigned long long g_phase2[4096][16];
 #define FFPP_PHASE(f, i) do { if (threadIdx.x == 0) g_phase[(f)][(i)] = gtimer(); } while (0)
+#define FFPP_PHASE2(f, i) do { if (threadIdx.x == 0) g_phase2[(f)][(i)] = gtimer(); } while (0)
 #else
 #define FFPP_PHASE(f, i) do { } while (0)
+#define FFPP_PHASE2(f, i) do { } while (0)
 #endif
 
 // ---- monotone float -> unsigned maps (descending: larger score -> smaller key) ----

@@ -324,6 +324,7 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
   const int n = surv_cnt[f * kCntStride];
   const int nsel = n < K ? n : K;
   const KeyT* gk = surv_keys + fd.cand_off;
+  FFPP_PHASE2(f, 0);
 
   // clear this frame's centroid histogram (uint16 per cell, two per word; boundary words are shared with the
   // neighbouring frames, which clear them too — every a2 CTA finishes before a4 counts)
@@ -335,6 +336,7 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
   }
 
   // ---- (1) threshold key = K-th smallest ----
+  FFPP_PHASE2(f, 1);
   KeyT thr = ~(KeyT)0;
   if (n > K) {
     KeyT prefix = 0, maskbits = 0;
@@ -387,6 +389,7 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
   }
 
   // ---- (2) gather the selected keys into shared memory: count per warp, scan the warps, then place (two sweeps
+  FFPP_PHASE2(f, 2);
   // over the L2-resident keys instead of one shared atomic per warp step on a single hot counter) ----
   {
     int mine = 0;
@@ -419,6 +422,7 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
   }
   for (int i = tid; i < K2_CNT_WORDS; i += K2_THREADS) cnt[i] = 0u;
   __syncthreads();
+  FFPP_PHASE2(f, 3);
 
   // ---- (3) decode (O1, O2) + spatial bin ----
   const int64_t obase = (int64_t)f * cst.kpad;
@@ -472,6 +476,7 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
     }
   }
   __syncthreads();
+  FFPP_PHASE2(f, 4);
 
   // ---- (4) exclusive scan of the bins (16 per thread), scatter to spatial order ----
   {
@@ -490,6 +495,7 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
     }
   }
   __syncthreads();
+  FFPP_PHASE2(f, 5);
   const uint16_t* base16 = reinterpret_cast<const uint16_t*>(cnt);
   for (int i0 = tid; i0 < nsel; i0 += 4 * K2_THREADS) {
     float4 box[4];
@@ -516,6 +522,11 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
       cellstart[(int64_t)f * kCellStride + ncells] = (uint16_t)nsel;      // ncells even or odd: the terminal entry
     }
   }
+#ifdef FFPP_PROFILE_PHASES
+  __syncthreads();
+  FFPP_PHASE2(f, 6);
+  if (tid == 0) g_phase2[f][7] = ((unsigned long long)n << 32) | (unsigned long long)nsel;
+#endif
 }
 
 // =====================================================================================================
