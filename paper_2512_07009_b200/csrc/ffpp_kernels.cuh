@@ -1210,12 +1210,28 @@ __global__ void __launch_bounds__(K4_THREADS, 2) k4_resolve_order(
   FFPP_PHASE(f, 4);
   if (bitonic) {
     k4_bitonic<KeyT>(kk, pp, kk1, pp1, m, Np, tid);
-  } else {
-    for (int shift = 0; shift < KB; shift += 8)
+  }
+  // LSD radix: a pass costs ~4 us per 3600 keys (shared-memory atomics and ballots), so only the SCORE half of the key is
+  // sorted; boxes of equal score are then put in candidate-index order by ranking inside their (short) tie group while the
+  // list is written out.  A tie group longer than 64 (thousands of equal logits: a degenerate input) takes the full-width
+  // sort instead.
+  constexpr int IB = KB / 2;                                   // index bits of the key: 16 / 32
+  bool tie_fix = false;
+  if (!bitonic) {
+    for (int shift = IB; shift < KB; shift += 8)
       if (k4_lsd_pass<KeyT>(kk, pp, kk1, pp1, m, shift, hist, misc, tid)) {
         KeyT* tk = kk; kk = kk1; kk1 = tk;
         uint16_t* tp = pp; pp = pp1; pp1 = tp;
       }
+    bool big = false;
+    for (int r = tid; r + 64 < m; r += K4_THREADS) big |= (kk[r] >> IB) == (kk[r + 64] >> IB);
+    tie_fix = !__syncthreads_or(big);
+    if (!tie_fix)
+      for (int shift = 0; shift < KB; shift += 8)
+        if (k4_lsd_pass<KeyT>(kk, pp, kk1, pp1, m, shift, hist, misc, tid)) {
+          KeyT* tk = kk; kk = kk1; kk1 = tk;
+          uint16_t* tp = pp; pp = pp1; pp1 = tp;
+        }
   }
   FFPP_PHASE(f, 5);
 
@@ -1224,7 +1240,22 @@ __global__ void __launch_bounds__(K4_THREADS, 2) k4_resolve_order(
   {
     KeyT* ok = kept_key + (int64_t)f * K;
     uint16_t* op = kept_pos + (int64_t)f * K;
-    for (int r = tid; r < m; r += K4_THREADS) { ok[r] = kk[r]; op[r] = pp[r]; }
+    if (!tie_fix) {
+      for (int r = tid; r < m; r += K4_THREADS) { ok[r] = kk[r]; op[r] = pp[r]; }
+    } else {
+      for (int r = tid; r < m; r += K4_THREADS) {
+        const KeyT key = kk[r], sc = key >> IB;
+        int g0 = r;
+        while (g0 > 0 && (kk[g0 - 1] >> IB) == sc) --g0;           // first element of the tie group (<= 64 long)
+        int rank = 0;
+        for (int j = g0; j < m; ++j) {
+          const KeyT kj = kk[j];
+          if ((kj >> IB) != sc) break;
+          rank += kj < key;                                        // equal score: the smaller candidate index comes first
+        }
+        ok[g0 + rank] = key; op[g0 + rank] = pp[r];
+      }
+    }
   }
 #ifdef FFPP_PROFILE_PHASES
   __syncthreads();
