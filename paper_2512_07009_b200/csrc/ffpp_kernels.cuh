@@ -799,7 +799,7 @@ constexpr int K4_WARPS = K4_THREADS / 32;
 constexpr int K4_SMEM_BUDGET = 108 * 1024;       // dynamic shared memory per CTA (two CTAs per SM)
 constexpr int K4_MAXPERM = 1024;                 // batches up to this many frames get the weight-ordered CTA -> frame map
 constexpr int K4_UNROLL = 8;
-constexpr int K4_BITONIC_MAX = 1024;             // kept sets up to this size take the bitonic network, larger ones LSD radix
+constexpr int K4_BITONIC_MAX = 256;              // kept sets up to this size take the bitonic network, larger ones LSD radix
 
 struct K4Misc {
   int wsum[K4_WARPS];
