@@ -210,11 +210,12 @@ int schedule(ffpp_handle* h, int B, const int32_t* N, const int32_t* dims, cudaS
     d.dens_off = cells;
     d.gw = W / p.cell_px; d.gh = H / p.cell_px;
     if (d.gw < R || d.gh < R) return fail(h, FFPP_EINVAL, "density grid smaller than the Gaussian radius");
-    int hs = 4;                                   // 16-pixel cells unless that needs more than 128 per axis
-    while ((128 << hs) < std::max(W, H)) ++hs;
-    d.hshift = hs;
+    // spatial cells 8 px wide x 16 px tall; both edges double until the frame has at most kMaxCells of them
+    int hs = 3, hsy = 4;
+    while ((int64_t)((W + (1 << hs) - 1) >> hs) * ((H + (1 << hsy) - 1) >> hsy) > kMaxCells) { if (hs < hsy) ++hs; else ++hsy; }
+    d.hshift = hs; d.hshift_y = hsy;
     d.cgw = (W + (1 << hs) - 1) >> hs;
-    d.cgh = (H + (1 << hs) - 1) >> hs;
+    d.cgh = (H + (1 << hsy) - 1) >> hsy;
     d.edge_off = edges;
     d.edge_cap = (int32_t)std::min<int64_t>(h->edges_per_box * d.nmax, 0x7fffffff);
     edges += d.edge_cap;

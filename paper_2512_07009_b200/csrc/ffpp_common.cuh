@@ -27,7 +27,9 @@ struct FrameDesc {
   int32_t W, H;                     // pixels
   int32_t nmax;                     // min(N, top_k): host-known bound on boxes entering NMS
   int32_t gw, gh;                   // density grid
-  int32_t hshift;                   // spatial cell = 2^hshift pixels
+  int32_t hshift;                   // spatial cell = 2^hshift pixels wide ...
+  int32_t hshift_y;                 // ... and 2^hshift_y pixels tall (8 x 16 when that fits kMaxCells: a window row is a
+                                    // contiguous range whatever its width in cells, so narrow cells trim it for free)
   int32_t cgw, cgh;                 // spatial cell grid (cgw * cgh <= kMaxCells), covers [0,W) x [0,H)
   int32_t lvl_start[kMaxLevels];    // first candidate of level l within the frame
   int32_t lvl_gw[kMaxLevels];       // W / s_l

@@ -426,7 +426,7 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
 
   // ---- (3) decode (O1, O2) + spatial bin ----
   const int64_t obase = (int64_t)f * cst.kpad;
-  const float cmx = (float)((fd.cgw << fd.hshift) - 1), cmy = (float)((fd.cgh << fd.hshift) - 1);
+  const float cmx = (float)((fd.cgw << fd.hshift) - 1), cmy = (float)((fd.cgh << fd.hshift_y) - 1);
   for (int i0 = tid; i0 < nsel; i0 += 4 * K2_THREADS) {
     float v[4][4];
     float ps[4][3];                                                // px, py, stride
@@ -467,7 +467,7 @@ __global__ void __launch_bounds__(K2_THREADS, 1) k2_select_bin(
         box.z = __fadd_rn(ps[u][0], __fmul_rn(v[u][2], s));
         box.w = __fadd_rn(ps[u][1], __fmul_rn(v[u][3], s));
         sel_box[obase + i] = box;
-        const uint32_t h = (uint32_t)(cell_coord(box_centre(box.y, box.w), cmy, fd.hshift) * fd.cgw +
+        const uint32_t h = (uint32_t)(cell_coord(box_centre(box.y, box.w), cmy, fd.hshift_y) * fd.cgw +
                                       cell_coord(box_centre(box.x, box.z), cmx, fd.hshift));
         const uint32_t sh = 16u * (h & 1u);
         const uint32_t old = atomicAdd(&cnt[h >> 1], 1u << sh);
@@ -585,7 +585,7 @@ __global__ void __launch_bounds__(K3_THREADS, 12) k3_nms_edges(const FrameDesc* 
   if (p0 + warp * 32 >= n) return;
   if (!kCount && *reinterpret_cast<volatile int*>(&frame_err[f])) return;   // the frame already goes to the overflow path
   const FrameDesc* fd = &frames[f];
-  const int cgw = fd->cgw, cgh = fd->cgh, hs = fd->hshift;
+  const int cgw = fd->cgw, cgh = fd->cgh, hs = fd->hshift, hsy = fd->hshift_y;
   const int64_t obase = (int64_t)f * cst.kpad;
   const float4* fbox = sp_box + obase;
   const KeyT* fkey = sp_key + obase;
@@ -602,13 +602,13 @@ __global__ void __launch_bounds__(K3_THREADS, 12) k3_nms_edges(const FrameDesc* 
   W.rowkey[lane] = fkey[pc];
 
   // window of cells that can hold a partner's centre
-  const float cmx = (float)((cgw << hs) - 1), cmy = (float)((cgh << hs) - 1);
+  const float cmx = (float)((cgw << hs) - 1), cmy = (float)((cgh << hsy) - 1);
   const float cxa = box_centre(a.x, a.z), cya = box_centre(a.y, a.w);
   const float ex = fmaxf(cst.rho * (a.z - a.x), 0.0f) * 1.001f + 1e-5f * (fabsf(a.x) + fabsf(a.z));
   const float ey = fmaxf(cst.rho * (a.w - a.y), 0.0f) * 1.001f + 1e-5f * (fabsf(a.y) + fabsf(a.w));
   const int Xlo = cell_coord(cxa - ex, cmx, hs), Xhi = cell_coord(cxa + ex, cmx, hs);
-  const int Ya = cell_coord(cya, cmy, hs);
-  const int Yhi = cell_coord(cya + ey, cmy, hs);
+  const int Ya = cell_coord(cya, cmy, hsy);
+  const int Yhi = cell_coord(cya + ey, cmy, hsy);
   int lcnt = 0, scnt = 0;                          // warp-uniform
   __syncwarp();
 
@@ -735,9 +735,9 @@ template <typename KeyT, int kThreads>
 __device__ __forceinline__ void overflow_fixed_point(uint8_t* state, const int n, const FrameDesc& fd, const float4* __restrict__ fbox,
                                                      const KeyT* __restrict__ fkey, const uint16_t* __restrict__ cs, const Consts& cst,
                                                      const int tid) {
-  const int cgw = fd.cgw, cgh = fd.cgh, hs = fd.hshift;
+  const int cgw = fd.cgw, cgh = fd.cgh, hs = fd.hshift, hsy = fd.hshift_y;
   volatile uint8_t* st = state;
-  const float cmx = (float)((cgw << hs) - 1), cmy = (float)((cgh << hs) - 1);
+  const float cmx = (float)((cgw << hs) - 1), cmy = (float)((cgh << hsy) - 1);
   for (;;) {
     bool undecided = false;
     for (int p = tid; p < n; p += kThreads) {
@@ -748,7 +748,7 @@ __device__ __forceinline__ void overflow_fixed_point(uint8_t* state, const int n
       const float ex = fmaxf(cst.rho * (a.z - a.x), 0.0f) * 1.001f + 1e-5f * (fabsf(a.x) + fabsf(a.z));
       const float ey = fmaxf(cst.rho * (a.w - a.y), 0.0f) * 1.001f + 1e-5f * (fabsf(a.y) + fabsf(a.w));
       const int Xlo = cell_coord(cxa - ex, cmx, hs), Xhi = cell_coord(cxa + ex, cmx, hs);
-      const int Ylo = cell_coord(cya - ey, cmy, hs), Yhi = cell_coord(cya + ey, cmy, hs);
+      const int Ylo = cell_coord(cya - ey, cmy, hsy), Yhi = cell_coord(cya + ey, cmy, hsy);
       bool removed = false, blocked = false;
       for (int Y = Ylo; Y <= Yhi && !removed; ++Y) {
         const uint16_t* r = cs + Y * cgw;
