@@ -29,7 +29,7 @@ __device__ __forceinline__ float load_prob(const __half* p, const int64_t i) { r
 // itself with its already-scanned foreground neighbours (left, up; up-left and up-right under 8-connectivity), a
 // union always hanging the LARGER root under the smaller one with atomicMin, so the root of a component is its
 // smallest index whatever the interleaving — the result is unique, hence deterministic and equal to the oracle's.
-//   kc_init    label = own index / -1, area counter = 0
+//   kc_init    label = first pixel of the row run inside the warp / -1, area counter of every self-labelled pixel = 0
 //   kc_merge   unions
 //   kc_flatten label = root; area[root] += 1
 //   kr_*       ordered compaction of the roots with area >= min_area into the table (ascending label); the table
@@ -65,7 +65,7 @@ __global__ void __launch_bounds__(KC_THREADS) kc_init(const T* __restrict__ src,
   const int first = 31 - __clz((int)(starts & (0xFFFFFFFFu >> (31 - lane))));
   if (valid) {
     labels[d.off + i] = fg ? i - (lane - first) : -1;
-    aux[d.off + i] = 0;
+    if (fg && first == lane) aux[d.off + i] = 0;             // only a pixel that labels itself can end up a root: its area counter
   }
   }
 }
