@@ -50,6 +50,8 @@ EXPORTS = ["ffpp_create", "ffpp_run", "ffpp_run_host", "ffpp_destroy", "ffpp_las
            "ffpp_set_stage_timing", "ffpp_get_stage_ms"]
 DEBUG_EXPORTS = ["ffpp_debug_read", "ffpp_debug_count_work", "ffpp_debug_stream_read"]     # include/ffpp_debug.h
 NEXT_EXPORTS = ["ffpp_heatmap_stats", "ffpp_density_exact", "ffpp_mask_components", "ffpp_preprocess"]   # include/ffpp_next.h
+NOALLOC_EXPORTS = ["ffpp_heatmap_entropy_noalloc"]                                                       # include/ffpp_noalloc.h
+NOALLOC_MAX_BLOCKS = 16384          # FFPP_NOALLOC_MAX_BLOCKS: B * ceil(gw*gh/2048) per call
 
 REGION_DTYPE = np.dtype([("label", "<i4"), ("area", "<i4"), ("x0", "<i4"), ("y0", "<i4"), ("x1", "<i4"), ("y1", "<i4"),
                          ("mass", "<f4"), ("reserved_", "<i4")])
@@ -82,7 +84,8 @@ class FFPPError(RuntimeError):
 
 def build(force: bool = False, verbose: bool = False) -> str:
     """Compile csrc/ffpp.cu for sm_100a into libffpp.so next to this file (nvcc cross-compiles without a GPU)."""
-    srcs = [os.path.join(_CSRC, s) for s in _SOURCES] + [os.path.join(_INCLUDE, "ffpp.h"), os.path.join(_INCLUDE, "ffpp_debug.h"), os.path.join(_INCLUDE, "ffpp_next.h")]
+    srcs = [os.path.join(_CSRC, s) for s in _SOURCES] + [os.path.join(_INCLUDE, "ffpp.h"), os.path.join(_INCLUDE, "ffpp_debug.h"), os.path.join(_INCLUDE, "ffpp_next.h"),
+                                                     os.path.join(_INCLUDE, "ffpp_noalloc.h")]
     stale = not os.path.exists(_LIB) or any(os.path.getmtime(s) > os.path.getmtime(_LIB) for s in srcs)
     if force or stale:
         cmd = ["nvcc"] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", _LIB, os.path.join(_CSRC, "ffpp.cu")]
@@ -131,6 +134,8 @@ def load_library() -> ctypes.CDLL:
         L.ffpp_mask_components.argtypes = [vp, vp, i32, i32, i32, i32, f32, i32, i32, i32, vp, vp, vp, vp]
         L.ffpp_preprocess.restype = ctypes.c_int
         L.ffpp_preprocess.argtypes = [vp, i32, i32, i32, i32, i32, vp, vp, i32, vp, vp]
+        L.ffpp_heatmap_entropy_noalloc.restype = ctypes.c_int
+        L.ffpp_heatmap_entropy_noalloc.argtypes = [vp, i32, i32, i32, vp, vp, vp]
         _lib = L
     return _lib
 
@@ -388,3 +393,17 @@ def preprocess(src, Hd: int, Wd: int, mean, std, *, out_dtype="fp16", stream=Non
     if rc != FFPP_OK:
         raise FFPPError(rc, "ffpp_preprocess")
     return dst
+
+
+def heatmap_entropy_noalloc(density, gw: int, gh: int, out_entropy, out_degree, stream=None) -> None:
+    """ffpp_heatmap_entropy_noalloc (include/ffpp_noalloc.h): density is a CUDA float32 tensor [B, gh, gw]; the two outputs
+    are caller-allocated CUDA float64 tensors [B].  The library allocates nothing (static 256 KiB device scratch)."""
+    import torch
+    lib = load_library()
+    assert density.is_cuda and density.dtype == torch.float32 and density.is_contiguous()
+    B = int(density.numel() // (gw * gh)) if gw > 0 and gh > 0 else 0
+    assert out_entropy.is_cuda and out_degree.is_cuda and out_entropy.dtype == torch.float64 and out_degree.dtype == torch.float64
+    st = stream if stream is not None else torch.cuda.current_stream()
+    rc = lib.ffpp_heatmap_entropy_noalloc(density.data_ptr(), B, gw, gh, st.cuda_stream, out_entropy.data_ptr(), out_degree.data_ptr())
+    if rc != FFPP_OK:
+        raise FFPPError(rc, lib.ffpp_last_error(None).decode())

@@ -819,3 +819,114 @@ int ffpp_debug_phases2(unsigned long long* dst, int frames) {
 }  // extern "C"
 
 #include "ffpp_next.cuh"
+
+// =====================================================================================================
+// The no-allocation entry point (include/ffpp_noalloc.h): entropy + clustering degree of B density grids of one size,
+// with the scratch of the partial sums in a file-scope device array instead of handle memory.  A variant of
+// ke_partial / ke_final (ffpp_next.cuh) for uniform grids: same block size, same per-thread cells, same summation order,
+// so the results equal ffpp_heatmap_stats' bit for bit.  Nothing here touches an existing code path.
+//
+// g_noalloc_scratch is a DEVICE array: in host code its name is only a host-side stand-in (passing it to a kernel would
+// fault or, where the GPU can reach host memory, silently use the wrong memory).  The host resolves its device address
+// with cudaGetSymbolAddress, once per device with that device current, and passes that pointer to the kernels.
+// =====================================================================================================
+#include <mutex>
+
+#include "../../include/ffpp_noalloc.h"
+
+static __device__ __align__(256) double2 g_noalloc_scratch[FFPP_NOALLOC_MAX_BLOCKS];   // 256 KiB per GPU, held until exit
+
+namespace ffpp {
+
+__global__ void __launch_bounds__(KE_THREADS) kn_entropy_partial(const float* __restrict__ D, int n, int nblk, double2* __restrict__ part) {
+  __shared__ double2 s_w[KE_THREADS / 32];
+  const int img = blockIdx.y;
+  const int base = blockIdx.x * KE_THREADS * KE_PER;          // grid.x == nblk: every (img, block) slot is written
+  const float* Df = D + (int64_t)img * n;
+  double a = 0.0, b = 0.0;
+#pragma unroll
+  for (int e = 0; e < KE_PER; ++e) {
+    const int i = base + e * KE_THREADS + threadIdx.x;
+    if (i < n) {
+      const float v = Df[i];
+      if (v > 0.0f) { const double dv = (double)v; a += dv; b += dv * log(dv); }
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) { a += __shfl_xor_sync(0xffffffffu, a, o); b += __shfl_xor_sync(0xffffffffu, b, o); }
+  if ((threadIdx.x & 31) == 0) s_w[threadIdx.x >> 5] = make_double2(a, b);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double2 t = make_double2(0.0, 0.0);
+    for (int wv = 0; wv < KE_THREADS / 32; ++wv) { t.x += s_w[wv].x; t.y += s_w[wv].y; }
+    part[(int64_t)img * nblk + blockIdx.x] = t;
+  }
+}
+
+__global__ void kn_entropy_final(int B, int n, int nblk, const double2* __restrict__ part, double* __restrict__ out_entropy,
+                                 double* __restrict__ out_degree) {
+  const int img = blockIdx.x * blockDim.x + threadIdx.x;
+  if (img >= B) return;
+  double a = 0.0, b = 0.0;
+  for (int k = 0; k < nblk; ++k) { const double2 t = part[(int64_t)img * nblk + k]; a += t.x; b += t.y; }
+  double H = 0.0, deg = 0.0;
+  if (a > 0.0) {
+    H = log(a) - b / a;
+    if (H < 0.0) H = 0.0;
+    if (n > 1) deg = 1.0 - H / log((double)n);
+  }
+  out_entropy[img] = H;
+  out_degree[img] = deg;
+}
+
+}  // namespace ffpp
+
+namespace {
+
+constexpr int kNoallocMaxDevices = 64;
+std::mutex g_noalloc_mu;
+double2* g_noalloc_ptr[kNoallocMaxDevices] = {};     // device address of g_noalloc_scratch, per device ordinal
+
+// device address of the scratch array on the CURRENT device (looked up once per device; no allocation)
+int noalloc_scratch(double2** out) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaGetDevice");
+  if (dev < 0 || dev >= kNoallocMaxDevices) return fail(nullptr, FFPP_ECAPACITY, "ffpp_heatmap_entropy_noalloc: device ordinal beyond 63");
+  std::lock_guard<std::mutex> lock(g_noalloc_mu);
+  if (!g_noalloc_ptr[dev]) {
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_noalloc_scratch);
+    if (e != cudaSuccess || !p) return cuda_fail(nullptr, e, "cudaGetSymbolAddress(g_noalloc_scratch)");
+    g_noalloc_ptr[dev] = static_cast<double2*>(p);
+  }
+  *out = g_noalloc_ptr[dev];
+  return FFPP_OK;
+}
+
+}  // namespace
+
+extern "C" int ffpp_heatmap_entropy_noalloc(const float* density, int32_t B, int32_t gw, int32_t gh, void* stream, double* out_entropy,
+                                            double* out_degree) {
+  using namespace ffpp;
+  if (B < 0) return fail(nullptr, FFPP_EINVAL, "ffpp_heatmap_entropy_noalloc: B < 0");
+  if (B == 0) return FFPP_OK;
+  if (!density || !out_entropy || !out_degree) return fail(nullptr, FFPP_EINVAL, "ffpp_heatmap_entropy_noalloc: null pointer");
+  if (gw < 1 || gh < 1 || (int64_t)gw * gh >= ((int64_t)1 << 31)) return fail(nullptr, FFPP_EINVAL, "ffpp_heatmap_entropy_noalloc: grid size out of range");
+  if (B > 65535) return fail(nullptr, FFPP_ECAPACITY, "ffpp_heatmap_entropy_noalloc: more than 65535 grids in one call");
+  const int n = gw * gh;
+  const int nblk = (n + KE_THREADS * KE_PER - 1) / (KE_THREADS * KE_PER);
+  if ((int64_t)B * nblk > FFPP_NOALLOC_MAX_BLOCKS)
+    return fail(nullptr, FFPP_ECAPACITY,
+                "ffpp_heatmap_entropy_noalloc: B * ceil(gw*gh/2048) = " + std::to_string((int64_t)B * nblk) + " exceeds the static scratch of " +
+                    std::to_string(FFPP_NOALLOC_MAX_BLOCKS) + " blocks (256 KiB); split the batch or use ffpp_heatmap_stats");
+  double2* scratch = nullptr;
+  const int rc = noalloc_scratch(&scratch);
+  if (rc != FFPP_OK) return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  kn_entropy_partial<<<dim3((unsigned)nblk, (unsigned)B), KE_THREADS, 0, st>>>(density, n, nblk, scratch);
+  kn_entropy_final<<<(B + 127) / 128, 128, 0, st>>>(B, n, nblk, scratch, out_entropy, out_degree);
+  const cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return cuda_fail(nullptr, e, "ffpp_heatmap_entropy_noalloc launch");
+  return FFPP_OK;
+}

@@ -24,7 +24,9 @@ def test_library_builds_loads_and_exports_the_header():
     assert not [s for s in syms if "debug" in s], "include/ffpp.h is the contract only"
     nxt = declared_symbols("ffpp_next.h")
     assert set(nxt) == set(m.NEXT_EXPORTS), (nxt, m.NEXT_EXPORTS)
-    for s in syms + dbg + nxt:
+    noa = declared_symbols("ffpp_noalloc.h")
+    assert set(noa) == set(m.NOALLOC_EXPORTS), (noa, m.NOALLOC_EXPORTS)
+    for s in syms + dbg + nxt + noa:
         assert hasattr(lib, s), f"libffpp.so does not export {s}"
     # null-handle calls that need no device
     lib.ffpp_destroy.argtypes = [ctypes.c_void_p]
